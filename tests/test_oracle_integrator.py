@@ -1,0 +1,193 @@
+"""Pins for oracle.rk4_step / correct / integrate (CPU only): textbook Kepler solution, invariants,
+reversibility, brute-force constrained minimisation, closed-form FLI growth.  DESIGN.md "Oracle pins"."""
+import numpy as np
+import pytest
+from scipy.optimize import minimize
+
+import oracle
+from conftest import random_states
+from paper_1802_00147_b200 import workloads
+
+
+def kepler_state(a, e, t):
+    """Textbook two-body solution (mu = 1) started at pericentre on the x axis, via Kepler's equation."""
+    n = a ** -1.5
+    M = n * t
+    E = M
+    for _ in range(60):
+        E = E - (E - e * np.sin(E) - M) / (1 - e * np.cos(E))
+    b = a * np.sqrt(1 - e * e)
+    x, y = a * (np.cos(E) - e), b * np.sin(E)
+    Edot = n / (1 - e * np.cos(E))
+    return np.array([x, y, 0.0, -a * np.sin(E) * Edot, b * np.cos(E) * Edot, 0.0])
+
+
+def kepler_z0(a, e):
+    z = np.zeros((12, 1))
+    z[0:6, 0] = kepler_state(a, e, 0.0)
+    z[8], z[11] = 1, 1
+    return z
+
+
+def test_rk4_reproduces_kepler_orbit_with_fourth_order_convergence():
+    a, e = 12.0, 0.3
+    T = 2 * np.pi * a ** 1.5
+    errs = []
+    for n_steps in (400, 800, 1600):
+        res = oracle.integrate(kepler_z0(a, e), T / n_steps, n_steps, mode=0, terms=0)
+        errs.append(np.abs(res.states[0:6, 0] - kepler_state(a, e, T)).max())
+    assert errs[0] < 2e-3 and errs[2] < 1e-5              # Kepler period: orbit closes after T
+    assert 13.0 < errs[0] / errs[1] < 19.0 and 13.0 < errs[1] / errs[2] < 19.0, errs  # global error ~ h^4
+    # a quarter period lands on the closed-form point too (not just periodicity)
+    res = oracle.integrate(kepler_z0(a, e), T / 6400, 1600, mode=0, terms=0)
+    assert np.abs(res.states[0:6, 0] - kepler_state(a, e, T / 4)).max() < 1e-8
+
+
+def test_single_rk4_step_local_error_is_fifth_order():
+    z = workloads.paper_orbit(2)
+    kw = dict(beta=1.0, chi1=1.0, chi2=1.0, terms=15)
+    ref = oracle.integrate(z.states, 1.0 / 64, 64, mode=0, **kw).states
+    e1 = np.abs(oracle.rk4_step(z.states, 1.0, **kw) - ref).max()
+    ref2 = oracle.integrate(z.states, 0.5 / 64, 64, mode=0, **kw).states
+    e2 = np.abs(oracle.rk4_step(z.states, 0.5, **kw) - ref2).max()
+    assert 24.0 < e1 / e2 < 40.0, (e1, e2)
+
+
+@pytest.mark.parametrize("which", [1, 2, 4])
+def test_correction_keeps_all_six_integrals_to_roundoff_on_the_papers_orbits(which):
+    """north_star: "conservation of every integral to round-off after correction"; Table 2
+     reports 1e-15 / 1e-11 for the corrected runs at t = 1e4."""
+    w = workloads.paper_orbit(which)
+    res = oracle.integrate(w.states, 1.0, 10_000, mode=3, **w.params())
+    i0, i1 = res.invariants[0:6, 0], res.invariants[6:12, 0]
+    assert res.status[0] == 0 and res.steps_done[0] == 10_000
+    assert abs(i1[0] - i0[0]) / abs(i0[0]) < 1e-14
+    assert np.linalg.norm(i1[1:4] - i0[1:4]) / np.linalg.norm(i0[1:4]) < 1e-14
+    assert abs(i1[4] - 1) < 1e-15 and abs(i1[5] - 1) < 1e-15
+    raw = oracle.integrate(w.states, 1.0, 10_000, mode=0, **w.params())
+    drift_raw = abs(raw.invariants[6, 0] - i0[0]) / abs(i0[0])
+    assert drift_raw > 1e-11                                # uncorrected RK4 really drifts
+
+
+@pytest.mark.parametrize("mode", [2, 3])
+def test_correction_operator_lands_on_the_manifold_and_is_idempotent(mode):
+    z0 = workloads.config0(16).states
+    kw = dict(beta=np.linspace(0.5, 1, 16), chi1=0.9, chi2=0.8, kq1=2.0, kq2=3.0, terms=31)
+    I0 = oracle.integrals(z0, **kw)
+    rng = np.random.default_rng(5)
+    zp = z0 + 1e-6 * rng.normal(size=z0.shape) * np.abs(z0).max(axis=1, keepdims=True)
+    zc, ok = oracle.correct(zp, I0[0], I0[1:4], mode, newton_iters=4, **kw)
+    assert ok.all()
+    I1 = oracle.integrals(zc, **kw)
+    assert np.abs(I1[0] / I0[0] - 1).max() < 1e-15
+    assert np.abs(I1[4:6] - 1).max() < 1e-15
+    if mode == 3:
+        assert (np.linalg.norm(I1[1:4] - I0[1:4], axis=0) / np.linalg.norm(I0[1:4], axis=0)).max() < 1e-15
+    else:
+        assert np.abs(np.linalg.norm(I1[1:4], axis=0) / np.linalg.norm(I0[1:4], axis=0) - 1).max() < 1e-15
+        # dual scaling only rescales: directions of r and p are untouched (eq 11)
+        for b in (0, 3):
+            c = (zc[b:b + 3] * zp[b:b + 3]).sum(0) / np.linalg.norm(zc[b:b + 3], axis=0) / np.linalg.norm(zp[b:b + 3], axis=0)
+            assert np.abs(c - 1).max() < 1e-15
+    zcc, _ = oracle.correct(zc, I0[0], I0[1:4], mode, newton_iters=4, **kw)
+    assert np.abs(zcc - zc).max() < 1e-14 * np.abs(zc).max()      # C(C(z)) = C(z)
+    z00, _ = oracle.correct(z0, I0[0], I0[1:4], mode, newton_iters=4, **kw)
+    assert np.abs(z00 - z0).max() < 1e-14 * np.abs(z0).max()      # C(z) = z on the manifold
+
+
+def test_mode1_only_normalises_spins():
+    z = random_states(4, seed=9)
+    z[6:12] *= 1.0 + 1e-3
+    zc, _ = oracle.correct(z, 0.0, np.zeros(3), 1)
+    assert np.array_equal(zc[0:6], z[0:6])
+    assert np.abs(np.linalg.norm(zc[6:9], axis=0) - 1).max() < 3e-16
+    assert np.abs(np.cross(zc[6:9].T, z[6:9].T)).max() < 1e-16
+
+
+def test_mode3_is_the_nearest_point_on_the_constraint_manifold():
+    """Brute force: minimise |dz|^2 over (r, p) subject to H = E0, r x p = J0 - S with SLSQP."""
+    z0 = workloads.paper_orbit(4).states
+    kw = dict(beta=1.0, chi1=1.0, chi2=1.0, terms=15)
+    I0 = oracle.integrals(z0, **kw)[:, 0]
+    zp = z0.copy()
+    zp[0:6, 0] += 1e-4 * np.array([1.0, -2.0, 0.5, 0.01, 0.02, -0.015])
+    zc, _ = oracle.correct(zp, I0[0], I0[1:4], 3, newton_iters=6, **kw)
+
+    def cons(x):
+        z = zp.copy()
+        z[0:6, 0] = x
+        I = oracle.integrals(z, **kw)[:, 0]
+        return np.array([(I[0] - I0[0]) * 1e3, *(I[1:4] - I0[1:4])])
+    sol = minimize(lambda x: 1e6 * np.sum((x - zp[0:6, 0]) ** 2), zp[0:6, 0], method="SLSQP",
+                   constraints=dict(type="eq", fun=cons), options=dict(ftol=1e-18, maxiter=200))
+    assert np.abs(cons(sol.x)).max() < 1e-10
+    d_oracle = np.linalg.norm(zc[0:6, 0] - zp[0:6, 0])
+    d_brute = np.linalg.norm(sol.x - zp[0:6, 0])
+    assert abs(d_oracle / d_brute - 1) < 1e-3                     # same distance to the manifold
+    assert np.abs(zc[0:6, 0] - sol.x).max() < 2e-3 * d_brute      # and (to second order) the same point
+
+
+def test_reversibility_of_a_regular_orbit_with_correction():
+    """N steps forward then N with -h returns to z0 within ~the global truncation error."""
+    w = workloads.paper_orbit(1)
+    fwd = oracle.integrate(w.states, 1.0, 2000, mode=3, **w.params())
+    back = oracle.integrate(fwd.states, -1.0, 2000, mode=3, **w.params())
+    fine = oracle.integrate(w.states, 0.25, 8000, mode=3, **w.params())
+    trunc = np.abs(fwd.states - fine.states).max()
+    assert np.abs(back.states - w.states).max() < 4 * trunc + 1e-12
+    assert trunc < 1e-4
+
+
+def test_fli_of_a_kepler_orbit_grows_like_log10_t():
+    """Regular motion: d(t) grows linearly ("power-law").  For a near-circular Kepler
+    orbit an offset eps in r changes a by 2 a^2 eps/r0^2 and the mean motion by -(3/2) da / a^(5/2):
+    d/d0 ~ 3 sqrt(a) t / r0^2."""
+    r0, f = 20.0, 0.97
+    z = np.zeros((12, 1))
+    z[0], z[4], z[8], z[11] = r0, f / np.sqrt(r0), 1, 1
+    a = -1 / (2 * (0.5 * z[4, 0] ** 2 - 1 / r0))
+    fli = {}
+    for t in (1000, 10_000, 100_000):
+        fli[t] = oracle.integrate(z, 1.0, t, mode=3, shadow_eps=1e-8, terms=0).fli[0]
+        assert abs(fli[t] - np.log10(3 * np.sqrt(a) * t / r0 ** 2)) < 0.15, (t, fli[t])
+    assert abs((fli[100_000] - fli[10_000]) - 1.0) < 0.05        # one unit per decade
+
+
+def test_fli_is_insensitive_to_renormalisation_interval_and_offset():
+    w = workloads.paper_orbit(1)
+    base = oracle.integrate(w.states, 1.0, 20_000, mode=3, shadow_eps=1e-8, **w.params()).fli[0]
+    other = oracle.integrate(w.states, 1.0, 20_000, mode=3, shadow_eps=1e-8, renorm_interval=1000, **w.params()).fli[0]
+    eps9 = oracle.integrate(w.states, 1.0, 20_000, mode=3, shadow_eps=1e-9, **w.params()).fli[0]
+    assert 1.0 < base < 5.0
+    assert abs(other - base) < 0.02 and abs(eps9 - base) < 0.05
+
+
+def test_status_codes_freeze_the_orbit_at_the_last_good_step():
+    z = np.zeros((12, 3))
+    z[0] = [6.0, 20.0, 20.0]
+    z[4] = [0.05, 0.9 / np.sqrt(20.0), 0.5]          # plunge, bound, hyperbolic
+    z[8], z[11] = 1, 1
+    res = oracle.integrate(z, 1.0, 3000, mode=3, shadow_eps=1e-8, r_merge=2.0, r_escape=200.0)
+    assert list(res.status) == [1, 0, 2]
+    assert res.steps_done[1] == 3000 and 0 < res.steps_done[0] < 3000 and 0 < res.steps_done[2] < 3000
+    r = np.linalg.norm(res.states[0:3], axis=0)
+    assert r[0] >= 2.0 and r[2] <= 200.0                # frozen before crossing
+    k = int(res.steps_done[0])                          # one more step would have crossed
+    again = oracle.integrate(z[:, :1], 1.0, k, mode=3, shadow_eps=1e-8, r_merge=0.0, r_escape=1e9)
+    assert np.array_equal(again.states[:, 0], res.states[:, 0])
+    nxt = oracle.integrate(z[:, :1], 1.0, k + 1, mode=3, shadow_eps=1e-8, r_merge=0.0, r_escape=1e9)
+    assert np.linalg.norm(nxt.states[0:3, 0]) < 2.0 or not np.isfinite(nxt.states).all()
+
+
+def test_double_and_long_double_oracles_agree():
+    w = workloads.config0(8)
+    a = oracle.integrate(w.states, 1.0, 1000, mode=3, **w.params())
+    b = oracle.integrate(w.states, 1.0, 1000, mode=3, precision=oracle.DOUBLE, **w.params())
+    rel = np.abs(a.states - b.states).max(axis=1) / np.abs(a.states).max(axis=1)
+    assert rel.max() < 1e-10
+
+
+def test_flop_counter_reports_the_oracles_own_formulation():
+    c = oracle.count_flops(workloads.paper_orbit(2).states[:, 0], terms=15, mode=3, newton_iters=2)
+    assert c["rk4_step"] == 4 * c["rhs"] + 159            # 3 stage inputs (3*25) + final combination (84)
+    assert 300 < c["rhs"] < 700 and c["correct"] > 2 * c["gradient"]

@@ -1,0 +1,294 @@
+#!/usr/bin/env python
+"""bench.py -- orbit-RK4-steps/s (with correction + FLI) on BASELINE config 2, and the FP64 roofline.
+
+One "step" = one pass of the whole hot path (mc_integrate: load, 1e5 x [RK4 + six-integral correction]
+on orbit and shadow, FLI renormalisation every 100 steps, status, store) over the 314 x 314 grid.
+N > 1 (torchrun): the global grid has 314*N rows of r0, sharded by contiguous row ranges, no
+collective on the data path (weak scaling).  `--impl reference` times the CPU oracle instead.
+Prints ONE JSON line on rank 0.  See DESIGN.md section 8 for every number's definition.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1802_00147_b200 import workloads  # noqa: E402
+
+METRIC = "orbit-RK4-steps/sec (with correction+FLI)"
+UNIT = "orbit-steps/s"
+# Algorithmic FP64 flops of one orbit-step (orbit + shadow, mode 3 with 2 Newton iterations, QM off),
+# FMA = 2, add/mul/rsqrt/rcp = 1: 2 x [4 x 229 (RHS) + 168 (RK4 sums) + 800 (correction) + 5 (|r|^2)].
+# Hand count of the kernel's own formulation, itemised in DESIGN.md section 6; the oracle's unfactored
+# formulation needs 8018 (oracle.count_flops), so this is the conservative figure.
+FLOP_PER_ORBIT_STEP = 3778.0
+FP64_LANES_PER_SM = 64
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="mc", choices=["mc", "reference"])
+    ap.add_argument("--grid", type=int, default=314, help="grid edge (314 = BASELINE config 2)")
+    ap.add_argument("--n-steps", type=int, default=100_000, help="RK4 steps per orbit (1e5 = config 2)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        return {}
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU every 100 ms (NVML) while the timed region runs."""
+    REASONS = {0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x10: "sync_boost",
+               0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown",
+               0x100: "display_clock_setting"}
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.mask, self.max_mhz, self.power = index, [], 0, None, []
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        while self.ok and not self._stop_evt.is_set():
+            try:
+                self.samples.append(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
+                self.mask |= int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                self.power.append(self.nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def stop(self):
+        self._stop_evt.set()
+        if self.is_alive():
+            self.join(timeout=2)
+        reasons = [n for b, n in self.REASONS.items() if self.mask & b]
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None, "sm_max_mhz": self.max_mhz,
+                "reasons": reasons, "power_w_max": max(self.power) if self.power else None,
+                "samples": len(self.samples)}
+
+
+def global_workload(args, world):
+    """Config 2 widened to 314*world rows of r0 (same r0 range, same theta axis)."""
+    return workloads.config2(n_r=args.grid * world, n_theta=args.grid, n_steps=args.n_steps)
+
+
+def rank_shard(w, args, rank, world):
+    lo, hi = workloads.shard_range(args.grid * world, rank, world)
+    return w.subset(np.arange(lo * args.grid, hi * args.grid))
+
+
+def cpu_baseline_sample(w, target_seconds=15.0):
+    """Time the oracle (double instance, all host cores) on a strided sample of the workload."""
+    import oracle
+    cores = oracle.max_threads()
+    n_probe = max(2 * cores, 16)
+    idx = np.linspace(0, w.n_orbits - 1, n_probe).astype(int)
+    sub = w.subset(idx)
+    t0 = time.perf_counter()
+    oracle.integrate(sub.states, w.h, 200, w.correction_mode, shadow_eps=w.shadow_eps, precision=oracle.DOUBLE,
+                     **sub.params())
+    rate = n_probe * 200 / (time.perf_counter() - t0)
+    steps = int(min(w.n_steps, 20_000))
+    n = int(max(cores, min(w.n_orbits, rate * target_seconds / steps)))
+    n = max(cores, (n // cores) * cores)
+    idx = np.linspace(0, w.n_orbits - 1, n).astype(int)
+    sub = w.subset(idx)
+    t0 = time.perf_counter()
+    oracle.integrate(sub.states, w.h, steps, w.correction_mode, shadow_eps=w.shadow_eps, precision=oracle.DOUBLE,
+                     **sub.params())
+    dt = time.perf_counter() - t0
+    return {"value": n * steps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{n} orbits strided over the grid x {steps} steps, double-precision instance of "
+                      f"oracle/pn_oracle.hpp, OpenMP static, {dt:.1f} s"}, (n, steps)
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores; rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = global_workload(args, 1)
+    base, (n, steps) = cpu_baseline_sample(w, target_seconds=8.0)
+    import oracle
+    idx = np.linspace(0, w.n_orbits - 1, n).astype(int)
+    sub = w.subset(idx)
+    times = []
+    for it in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        oracle.integrate(sub.states, w.h, steps, w.correction_mode, shadow_eps=w.shadow_eps,
+                         precision=oracle.DOUBLE, **sub.params())
+        if it >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    total = sum(times)
+    value = n * steps * args.steps / total
+    base["value"] = value
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"config2: {args.grid}x{args.grid} orbit scan, RK4 h=1, shadow 1e-8 + FLI, "
+                                   f"six-integral correction; each step = bounded sample ({n} orbits x {steps} steps)"},
+            "cpu_baseline": base,
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_mc(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1802_00147_b200 import binding
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = rank_shard(global_workload(args, world), args, rank, world)
+    n = w.n_orbits
+    orbit_steps_rank = float(n) * w.n_steps
+    z_dev = torch.as_tensor(w.states, device=dev)
+    z_pin = torch.as_tensor(w.states).pin_memory()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
+
+    peak_tf, peak_clock = binding.fp64_peak(local, 200.0) if rank == 0 else (None, None)
+    I = binding.Integrator(terms=w.terms, device=local)
+    out = torch.empty_like(z_dev)
+    stream = torch.cuda.current_stream(dev)
+    launches = 0
+
+    def one_step():
+        nonlocal launches
+        res = I.integrate(z_dev, w.h, w.n_steps, w.correction_mode, shadow_eps=w.shadow_eps, out_states=out)
+        launches += 1
+        return res
+
+    for _ in range(args.warmup):
+        one_step()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    launches = 0
+    barrier()
+    t_wall0 = time.perf_counter()
+    res = None
+    for k in range(args.steps):
+        flush.zero_()                                   # flush L2 between timed iterations
+        ev[k][0].record(stream)
+        res = one_step()
+        ev[k][1].record(stream)
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    clocks = sampler.stop()
+    kernel_ms = [a.elapsed_time(b) for a, b in ev]
+    dev_ms = float(sum(kernel_ms))
+    t = torch.tensor([dev_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dev_ms_max = float(t.item())
+    value = orbit_steps_rank * world * args.steps / (dev_ms_max * 1e-3)
+
+    # end to end through the C ABI with HOST buffers (pinned): H2D + kernel + D2H inside the timed call
+    z_host = z_pin.numpy()
+    I.integrate_host(z_host, w.h, min(w.n_steps, 100), w.correction_mode, shadow_eps=w.shadow_eps)   # warm scratch
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        hres = I.integrate_host(z_host, w.h, w.n_steps, w.correction_mode, shadow_eps=w.shadow_eps)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_value = orbit_steps_rank * world * args.steps / float(t.item())
+    h2d = 12 * 8 * n
+    d2h = (12 + 12 + 1) * 8 * n + 4 * n + 8 * n
+
+    info = I.launch_info()
+    status = res.status.cpu().numpy()
+    fli = res.fli.cpu().numpy()
+    I.close()
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    mp = measured_peaks()
+    sm_max = float(mp.get("sm_max_mhz", clocks.get("sm_max_mhz") or 1965.0))
+    nominal_tf = info["num_sms"] * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    per_launch_s = (dev_ms / args.steps) * 1e-3
+    achieved_tf = FLOP_PER_ORBIT_STEP * orbit_steps_rank / per_launch_s / 1e12
+    roofline = {"bound": "alu", "achieved": achieved_tf, "peak": nominal_tf, "unit": "TFLOP/s",
+                "frac": achieved_tf / nominal_tf, "traffic": None,
+                "peak_source": f"derived: {info['num_sms']} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x {sm_max:.0f} MHz "
+                               "(MEASURED_PEAKS.json has no FP64 entry)",
+                "peak_measured_dfma": peak_tf, "frac_of_measured_dfma": achieved_tf / peak_tf if peak_tf else None,
+                "dfma_probe_implied_sm_mhz": peak_clock,
+                "flop_per_orbit_step": FLOP_PER_ORBIT_STEP, "kernel": "mc::integrate_kernel<uniform,QM off,mode 3>",
+                "kernel_ms_per_launch": dev_ms / args.steps,
+                "regs_per_thread": info["regs_per_thread"], "spill_bytes": info["local_bytes"],
+                "blocks_per_sm": info["blocks_per_sm"], "grid": info["grid"], "block": info["block"]}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"config2: {args.grid}x{args.grid} orbit scan per GPU (r0 in [10,60] x theta in [0,pi]), "
+                                   f"equal mass, chi=1, N+1PN+2PN+SO+SS, RK4 h=1, {w.n_steps} steps, shadow 1e-8 "
+                                   "renormalised every 100 steps + FLI, six-integral correction (mode 3, 2 Newton iterations)",
+                       "orbits_per_gpu": n, "rk4_steps": w.n_steps, "l2": "flushed (256 MiB write) between timed iterations",
+                       "parallelism": f"orbit-sharded x{world}, no collective"},
+            "clocks": clocks, "wall_s_timed_region": t_wall,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+            "gpu_launches": launches, "roofline": roofline,
+            "outcome": {"regular": int(((status == 0) & (fli < 5.8)).sum()), "chaotic": int(((status == 0) & (fli >= 5.8)).sum()),
+                        "dropped": int((status != 0).sum()), "near_threshold": int(((status == 0) & (np.abs(fli - 5.8) < 0.5)).sum())}}
+    if not args.no_cpu_baseline:
+        line["cpu_baseline"], _ = cpu_baseline_sample(w)
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_mc(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,162 @@
+/* mc.h -- C ABI of libmc: batched manifold-corrected RK4 integration of the conservative PN
+ * Hamiltonian of spinning compact binaries on one NVIDIA B200 (sm_100a), FP64 throughout.
+ *
+ * Method: arXiv 1802.00147 (cited below as PAPER.md:<line>, the text under /root/reference at build
+ * time) as read in DESIGN.md (cited as DESIGN.md Rn).  No C++ types and no exceptions cross this
+ * boundary; every function returns 0 (MC_OK) or a negative mc_error.  There is no CPU fallback.
+ *
+ * Data layout (all entry points): one orbit's state is z = (r, p, S1hat, S2hat), 12 doubles
+ * (PAPER.md:81, 120): r in units of M, p in units of mu, unit spin vectors; G = c = M = 1.  A batch
+ * is structure-of-arrays, double[12][n_orbits], row c holds component c of every orbit in the order
+ * rx ry rz px py pz s1x s1y s1z s2x s2y s2z.
+ */
+#ifndef MC_H_
+#define MC_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mc_handle mc_handle; /* opaque; created by mc_create, freed by mc_destroy */
+
+enum mc_error {
+  MC_OK = 0,
+  MC_EINVAL = -1,  /* null pointer, negative size, unknown mode/term bit, beta outside (0,1], ... */
+  MC_ECUDA = -2,   /* a CUDA runtime call failed; mc_strerror(MC_ECUDA) returns the CUDA message  */
+  MC_EARCH = -3,   /* the device is not compute capability 10.x (the library holds sm_100a code only) */
+  MC_ENOMEM = -4   /* host allocation failed */
+};
+
+/* Hamiltonian terms, eq (1) of the paper.  H_N is always on. */
+enum mc_terms {
+  MC_TERM_1PN = 1u,   /* H_1PN (ADM; R1)                        */
+  MC_TERM_2PN = 2u,   /* H_2PN                                            */
+  MC_TERM_SO = 4u,    /* spin-orbit, L-terms of eqs (8)-(9) */
+  MC_TERM_S1S2 = 8u,  /* eq (3)                              */
+  MC_TERM_QM = 16u    /* eqs (4)-(5), quadrupole-monopole */
+};
+
+/* Correction applied after every RK4 step. */
+enum mc_correction {
+  MC_CORR_NONE = 0,      /* plain RK4                                                             */
+  MC_CORR_SPINS = 1,     /* eq (10): S_i_hat <- S_i_hat / |S_i_hat|                                 */
+  MC_CORR_DUAL = 2,      /* eq (10) + the paper's dual scaling p <- alpha p, r <- beta r, eqs (11)-(13):
+                            exact H = E0 and |J| = |J0|                                            */
+  MC_CORR_SIXINT = 3     /* eq (10) + minimal-norm projection of (r,p) onto H = E0, J = J0 (vector):
+                            all six integrals to round-off (R4); "correction on"         */
+};
+
+/* Per-orbit outcome (merged / unbound orbits are dropped; R13). */
+enum mc_status {
+  MC_ST_OK = 0,
+  MC_ST_MERGED = 1,     /* |r| < r_merge after a step; state frozen at the last good step */
+  MC_ST_UNBOUND = 2,    /* |r| > r_escape                                                   */
+  MC_ST_NONFINITE = 3,  /* a non-finite component in the orbit or its shadow                */
+  MC_ST_NEWTON_FLAG = 256 /* OR-ed in: mode 2 skipped its (r,p) scaling on >= 1 step (R7) */
+};
+
+typedef struct mc_params {
+  uint32_t struct_size;   /* = sizeof(mc_params); checked by mc_create                                   */
+  uint32_t terms;         /* OR of mc_terms                                                              */
+  int32_t device;         /* CUDA device ordinal                                                         */
+  int32_t per_orbit;      /* 0: the five scalars below apply to every orbit; 1: use the device arrays      */
+  double beta;            /* mass ratio m1/m2 in (0,1]                                       */
+  double chi1, chi2;      /* dimensionless spins in [0,1]                                   */
+  double kq1, kq2;        /* quadrupole coefficients, 1 = black hole (R16)         */
+  const double* d_beta;   /* per_orbit = 1: DEVICE arrays of length >= n_orbits, owned by the caller,      */
+  const double* d_chi1;   /*   must stay valid until mc_destroy; values are not validated on the device    */
+  const double* d_chi2;
+  const double* d_kq1;
+  const double* d_kq2;
+  int32_t renorm_interval; /* steps between shadow renormalisations, > 0 (BASELINE config 1: 100)          */
+  int32_t newton_iters;    /* fixed Newton iteration count, 1..16 (R6); default 2                */
+  double newton_tol;       /* epsilon of PAPER.md:197 (1e-10): mode 2 convergence test on |dv|             */
+  double r_merge;          /* default 2    (R13)                                                 */
+  double r_escape;         /* default 1e4                                                                  */
+  void* cuda_stream;       /* cudaStream_t all work is enqueued on (e.g. torch's current stream); NULL = 0 */
+} mc_params;
+
+/* Fill *p with defaults: terms = 1PN|2PN|SO|S1S2, device 0, uniform beta = chi = kq = 1,
+ * renorm_interval 100, newton_iters 2, newton_tol 1e-10, r_merge 2, r_escape 1e4, stream NULL. */
+int mc_params_default(mc_params* p);
+
+/* Validate params, select the device, allocate the handle.  *out_handle is set only on success. */
+int mc_create(const mc_params* params, mc_handle** out_handle);
+
+/* Integrate n_orbits independent orbits for n_steps classical RK4 steps of size step_h (may be
+ * negative), applying correction_mode after every step (the per-orbit algorithm
+ * is spelled out in DESIGN.md section 2).  Reference integrals E0, J0 are taken from the input states
+ * (PAPER.md:136); with correction_mode >= 1 the input spins are normalised first.
+ *
+ * shadow_eps != 0 adds, per orbit, a shadow trajectory started at rx + shadow_eps, integrated and
+ * corrected onto its own integrals, renormalised to distance |shadow_eps| every renorm_interval
+ * steps, and writes the fast Lyapunov indicator FLI = log10(d(t)/d(0)) (R10-R12).
+ *
+ *   states          DEVICE, const double[12][n_orbits]                       (read)
+ *   out_states      DEVICE, double[12][n_orbits], may alias states            (written)
+ *   out_invariants  DEVICE, double[12][n_orbits] or NULL: rows 0-5 = E, Jx, Jy, Jz, |S1hat|, |S2hat| of
+ *                   the (normalised) input state, rows 6-11 = the same of the output state
+ *   out_fli         DEVICE, double[n_orbits]; required iff shadow_eps != 0
+ *
+ * The call is asynchronous on params.cuda_stream: one kernel launch, no host synchronisation, no
+ * host<->device copy.  All buffers are owned by the caller.  n_orbits = 0 or n_steps = 0 are valid
+ * (n_steps = 0 copies the normalised state and evaluates the invariants).  Numerical failures of
+ * single orbits are not errors: see mc_get_status.
+ * Errors: MC_EINVAL (null/negative arguments, unknown mode, non-finite step_h), MC_ECUDA. */
+int mc_integrate(mc_handle* h, const double* states, int64_t n_orbits, double step_h, int64_t n_steps,
+                 int32_t correction_mode, double shadow_eps, double* out_states,
+                 double* out_invariants, double* out_fli);
+
+/* Same operation with HOST buffers (pageable or pinned): copies the inputs to device scratch owned by
+ * the handle, runs mc_integrate, copies the outputs back and synchronises the stream before
+ * returning.  out_status (int32[n_orbits]) and out_step (int64[n_orbits]) are optional host arrays. */
+int mc_integrate_host(mc_handle* h, const double* states, int64_t n_orbits, double step_h,
+                      int64_t n_steps, int32_t correction_mode, double shadow_eps, double* out_states,
+                      double* out_invariants, double* out_fli, int32_t* out_status, int64_t* out_step);
+
+/* Status of the orbits of the most recent mc_integrate on this handle, copied (stream-ordered) into
+ * DEVICE arrays of the caller: out_status int32[n_orbits] (mc_status), out_step int64[n_orbits] =
+ * number of completed steps.  Either pointer may be NULL. */
+int mc_get_status(mc_handle* h, int32_t* out_status, int64_t* out_step);
+
+/* Evaluate pieces of the model on the device with the handle's parameters (used by the parity tests
+ * to compare the kernel's fused routines with the oracle one by one).  states: DEVICE double[12][n].
+ *   what = 0: out[1][n]  = H                     (eq 1)
+ *   what = 1: out[12][n] = dz/dt                 (eqs 6-9: dH/dp, -dH/dr, Omega_i x S_i_hat)
+ *   what = 2: out[6][n]  = E, Jx, Jy, Jz, |S1hat|, |S2hat|
+ *   what = 3: out[12][n] = one RK4 step of size step_h, no correction
+ *   what = 4: out[12][n] = correction operator of mode `mode` applied to states, with references
+ *             refs = DEVICE double[4][n] (E0, J0x, J0y, J0z)
+ * Asynchronous on the handle's stream. */
+int mc_eval(mc_handle* h, int32_t what, const double* states, int64_t n, double step_h, int32_t mode,
+            const double* refs, double* out);
+
+/* Facts about the kernel the last mc_integrate launched (for bench.py / DESIGN.md evidence). */
+typedef struct mc_launch_info {
+  int32_t grid, block;          /* launch shape                                   */
+  int32_t regs_per_thread;      /* cudaFuncAttributes.numRegs                     */
+  int32_t local_bytes;          /* cudaFuncAttributes.localSizeBytes (spills)     */
+  int32_t blocks_per_sm;        /* occupancy API result for that block size       */
+  int32_t num_sms;
+  int32_t smem_bytes;           /* dynamic shared memory per block                */
+  int32_t variant;              /* bit0 per-orbit params, bit1 QM, bits 4-5 mode  */
+  int64_t trajectories;         /* threads doing work = n_orbits * (1 + shadow)   */
+} mc_launch_info;
+int mc_last_launch_info(mc_handle* h, mc_launch_info* out);
+
+/* DFMA throughput of the device, measured: every SM runs independent FMA chains for about
+ * `millis` ms; *out_tflops = 2 * FMAs / time (CUDA events).  The roofline denominator of bench.py
+ * (MEASURED_PEAKS.json has no FP64 entry).  Synchronous. */
+int mc_fp64_peak(int32_t device, double millis, double* out_tflops, double* out_sm_clock_mhz);
+
+int mc_destroy(mc_handle* h);
+
+/* Static string for an mc_error; for MC_ECUDA the text of the last CUDA error seen by this thread. */
+const char* mc_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MC_H_ */

@@ -1,0 +1,225 @@
+"""Thin Python binding of libmc.so (include/mc.h): argument marshalling only.
+
+torch is used for device memory and streams; every step of the path runs in the CUDA kernels behind
+the C ABI.  There is no CPU fallback: if the library cannot be loaded or built, import of the symbols
+fails loudly (MCLibraryError).
+"""
+import ctypes
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+from . import build as _build
+
+MC_TERM_1PN, MC_TERM_2PN, MC_TERM_SO, MC_TERM_S1S2, MC_TERM_QM = 1, 2, 4, 8, 16
+TERMS_DEFAULT = MC_TERM_1PN | MC_TERM_2PN | MC_TERM_SO | MC_TERM_S1S2
+MC_OK, MC_EINVAL, MC_ECUDA, MC_EARCH, MC_ENOMEM = 0, -1, -2, -3, -4
+
+# every symbol include/mc.h declares (tests/test_abi.py checks the header against this list)
+EXPORTS = ["mc_params_default", "mc_create", "mc_integrate", "mc_integrate_host", "mc_get_status", "mc_eval",
+           "mc_last_launch_info", "mc_fp64_peak", "mc_destroy", "mc_strerror"]
+
+
+class MCLibraryError(RuntimeError):
+    pass
+
+
+class MCError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libmc error {code}: {msg}")
+        self.code = code
+
+
+class mc_params(ctypes.Structure):
+    _fields_ = [("struct_size", ctypes.c_uint32), ("terms", ctypes.c_uint32), ("device", ctypes.c_int32),
+                ("per_orbit", ctypes.c_int32), ("beta", ctypes.c_double), ("chi1", ctypes.c_double),
+                ("chi2", ctypes.c_double), ("kq1", ctypes.c_double), ("kq2", ctypes.c_double),
+                ("d_beta", ctypes.c_void_p), ("d_chi1", ctypes.c_void_p), ("d_chi2", ctypes.c_void_p),
+                ("d_kq1", ctypes.c_void_p), ("d_kq2", ctypes.c_void_p), ("renorm_interval", ctypes.c_int32),
+                ("newton_iters", ctypes.c_int32), ("newton_tol", ctypes.c_double), ("r_merge", ctypes.c_double),
+                ("r_escape", ctypes.c_double), ("cuda_stream", ctypes.c_void_p)]
+
+
+class mc_launch_info(ctypes.Structure):
+    _fields_ = [("grid", ctypes.c_int32), ("block", ctypes.c_int32), ("regs_per_thread", ctypes.c_int32),
+                ("local_bytes", ctypes.c_int32), ("blocks_per_sm", ctypes.c_int32), ("num_sms", ctypes.c_int32),
+                ("smem_bytes", ctypes.c_int32), ("variant", ctypes.c_int32), ("trajectories", ctypes.c_int64)]
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def load_library():
+    """dlopen libmc.so (building it with nvcc first if it is missing or stale). Never falls back."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    try:
+        path = _build.build()
+    except Exception as e:  # nvcc missing or compile error
+        if os.path.exists(_build.LIB):
+            path = _build.LIB
+        else:
+            raise MCLibraryError(f"libmc.so is not built and could not be built: {e}") from e
+    try:
+        lib = ctypes.CDLL(path)
+    except OSError as e:
+        raise MCLibraryError(f"cannot load {path}: {e}") from e
+    vp, i32, i64, dbl = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_double
+    lib.mc_params_default.argtypes = [ctypes.POINTER(mc_params)]
+    lib.mc_create.argtypes = [ctypes.POINTER(mc_params), ctypes.POINTER(vp)]
+    lib.mc_integrate.argtypes = [vp, vp, i64, dbl, i64, i32, dbl, vp, vp, vp]
+    lib.mc_integrate_host.argtypes = [vp, vp, i64, dbl, i64, i32, dbl, vp, vp, vp, vp, vp]
+    lib.mc_get_status.argtypes = [vp, vp, vp]
+    lib.mc_eval.argtypes = [vp, i32, vp, i64, dbl, i32, vp, vp]
+    lib.mc_last_launch_info.argtypes = [vp, ctypes.POINTER(mc_launch_info)]
+    lib.mc_fp64_peak.argtypes = [i32, dbl, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
+    lib.mc_destroy.argtypes = [vp]
+    lib.mc_strerror.argtypes = [ctypes.c_int]
+    lib.mc_strerror.restype = ctypes.c_char_p
+    for name in EXPORTS:
+        if name != "mc_strerror":
+            getattr(lib, name).restype = ctypes.c_int
+    _lib = lib
+    return lib
+
+
+def _check(rc):
+    if rc != MC_OK:
+        raise MCError(rc, load_library().mc_strerror(rc).decode())
+
+
+def params_default() -> mc_params:
+    p = mc_params()
+    _check(load_library().mc_params_default(ctypes.byref(p)))
+    return p
+
+
+def fp64_peak(device: int = 0, millis: float = 200.0):
+    """(TFLOP/s, implied SM clock in MHz) of the DFMA probe in libmc."""
+    t, c = ctypes.c_double(), ctypes.c_double()
+    _check(load_library().mc_fp64_peak(device, millis, ctypes.byref(t), ctypes.byref(c)))
+    return t.value, c.value
+
+
+@dataclass
+class IntegrateResult:
+    states: "object"                 # torch.Tensor (12, n) float64, device
+    invariants: Optional["object"]   # (12, n) or None
+    fli: Optional["object"]          # (n,) or None
+    status: "object"                 # (n,) int32
+    steps_done: "object"             # (n,) int64
+
+
+class Integrator:
+    """mc_create / mc_integrate / mc_destroy with torch tensors as device buffers."""
+
+    def __init__(self, terms=TERMS_DEFAULT, beta=1.0, chi1=1.0, chi2=1.0, kq1=1.0, kq2=1.0, device=0,
+                 renorm_interval=100, newton_iters=2, newton_tol=1e-10, r_merge=2.0, r_escape=1e4, stream=None):
+        import torch
+        self._torch = torch
+        self._lib = load_library()
+        p = params_default()
+        p.terms, p.device = int(terms), int(device)
+        p.renorm_interval, p.newton_iters, p.newton_tol = int(renorm_interval), int(newton_iters), float(newton_tol)
+        p.r_merge, p.r_escape = float(r_merge), float(r_escape)
+        self.device = torch.device("cuda", device)
+        vals = dict(beta=beta, chi1=chi1, chi2=chi2, kq1=kq1, kq2=kq2)
+        per_orbit = any(hasattr(v, "__len__") for v in vals.values())
+        self._keep = []
+        self.n_params = None
+        if per_orbit:
+            n = max(len(v) for v in vals.values() if hasattr(v, "__len__"))
+            self.n_params = n
+            p.per_orbit = 1
+            for name, v in vals.items():
+                t = torch.as_tensor(v, dtype=torch.float64).expand(n).contiguous().to(self.device)
+                self._keep.append(t)            # must outlive the handle (include/mc.h)
+                setattr(p, "d_" + name, t.data_ptr())
+        else:
+            for name, v in vals.items():
+                setattr(p, name, float(v))
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device)
+        self.stream = stream
+        p.cuda_stream = stream.cuda_stream
+        self.params = p
+        self._h = ctypes.c_void_p()
+        _check(self._lib.mc_create(ctypes.byref(p), ctypes.byref(self._h)))
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.mc_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    __del__ = close
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def _dev(self, x):
+        torch = self._torch
+        t = torch.as_tensor(x, dtype=torch.float64)
+        if t.device != self.device:
+            t = t.to(self.device)
+        return t.contiguous()
+
+    def integrate(self, states, h, n_steps, correction_mode=3, shadow_eps=0.0, want_invariants=True,
+                  out_states=None) -> IntegrateResult:
+        """states: (12, n) float64 (device tensor, or anything torch.as_tensor accepts)."""
+        torch = self._torch
+        z = self._dev(states)
+        assert z.dim() == 2 and z.shape[0] == 12, z.shape
+        n = z.shape[1]
+        if self.n_params is not None and n > self.n_params:
+            raise ValueError("more orbits than per-orbit parameters")
+        out = torch.empty_like(z) if out_states is None else out_states
+        inv = torch.empty_like(z) if want_invariants else None
+        fli = torch.empty(n, dtype=torch.float64, device=self.device) if shadow_eps != 0.0 else None
+        _check(self._lib.mc_integrate(self._h, z.data_ptr(), n, float(h), int(n_steps), int(correction_mode),
+                                      float(shadow_eps), out.data_ptr(), inv.data_ptr() if inv is not None else None,
+                                      fli.data_ptr() if fli is not None else None))
+        status = torch.empty(n, dtype=torch.int32, device=self.device)
+        steps = torch.empty(n, dtype=torch.int64, device=self.device)
+        _check(self._lib.mc_get_status(self._h, status.data_ptr(), steps.data_ptr()))
+        return IntegrateResult(out, inv, fli, status, steps)
+
+    def integrate_host(self, states_np, h, n_steps, correction_mode=3, shadow_eps=0.0):
+        """mc_integrate_host: numpy (host) in, numpy out; copies are inside the call."""
+        import numpy as np
+        z = np.ascontiguousarray(states_np, dtype=np.float64)
+        n = z.shape[1]
+        out, inv = np.empty_like(z), np.empty_like(z)
+        fli = np.empty(n) if shadow_eps != 0.0 else None
+        status, steps = np.empty(n, dtype=np.int32), np.empty(n, dtype=np.int64)
+        _check(self._lib.mc_integrate_host(self._h, z.ctypes.data, n, float(h), int(n_steps), int(correction_mode),
+                                           float(shadow_eps), out.ctypes.data, inv.ctypes.data,
+                                           fli.ctypes.data if fli is not None else None, status.ctypes.data,
+                                           steps.ctypes.data))
+        return IntegrateResult(out, inv, fli, status, steps)
+
+    _WHAT = {"H": (0, 1), "rhs": (1, 12), "integrals": (2, 6), "rk4_step": (3, 12), "correct": (4, 12)}
+
+    def eval(self, what, states, h=0.0, mode=0, refs=None):
+        """mc_eval: what in {"H","rhs","integrals","rk4_step","correct"} -> tensor (rows, n)."""
+        torch = self._torch
+        z = self._dev(states)
+        n = z.shape[1]
+        code, rows = self._WHAT[what]
+        out = torch.empty((rows, n), dtype=torch.float64, device=self.device)
+        r = self._dev(refs) if refs is not None else None
+        _check(self._lib.mc_eval(self._h, code, z.data_ptr(), n, float(h), int(mode),
+                                 r.data_ptr() if r is not None else None, out.data_ptr()))
+        return out
+
+    def launch_info(self) -> dict:
+        info = mc_launch_info()
+        _check(self._lib.mc_last_launch_info(self._h, ctypes.byref(info)))
+        return {k: getattr(info, k) for k, _ in mc_launch_info._fields_}

@@ -1,0 +1,374 @@
+// mc_api.cu -- the C ABI of include/mc.h: handle, validation, launches, host-buffer variant,
+// evaluation entry point for the parity tests, FP64 peak probe.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "../../include/mc.h"
+#include "mc_kernel.cuh"
+#include "mc_launch.h"
+
+namespace {
+
+thread_local char g_cuda_msg[256] = "no CUDA error recorded";
+
+int cuda_fail(cudaError_t e) {
+  snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error %d: %s", (int)e, cudaGetErrorString(e));
+  return MC_ECUDA;
+}
+#define MC_CUDA(call)                               \
+  do {                                              \
+    cudaError_t e_ = (call);                        \
+    if (e_ != cudaSuccess) return cuda_fail(e_);    \
+  } while (0)
+
+struct DeviceBuf {
+  void* p = nullptr;
+  size_t cap = 0;
+  int reserve(size_t bytes) {
+    if (bytes <= cap) return MC_OK;
+    if (p) cudaFree(p);
+    p = nullptr;
+    cap = 0;
+    cudaError_t e = cudaMalloc(&p, bytes);
+    if (e != cudaSuccess) return cuda_fail(e);
+    cap = bytes;
+    return MC_OK;
+  }
+  void release() {
+    if (p) cudaFree(p);
+    p = nullptr;
+    cap = 0;
+  }
+};
+
+}  // namespace
+
+struct mc_handle {
+  mc_params P;
+  McConsts uc;               // derived constants of the uniform parameter set
+  cudaStream_t stream;
+  int num_sms;
+  int64_t last_n;            // orbits of the last mc_integrate (status buffers valid for these)
+  DeviceBuf status, step;    // int32[n], int64[n]
+  DeviceBuf h_in, h_out, h_inv, h_fli;   // scratch of mc_integrate_host
+  mc_launch_info info;
+};
+
+namespace {
+
+int valid_scalars(double beta, double chi1, double chi2, double kq1, double kq2) {
+  if (!(beta > 0.0) || !(beta <= 1.0)) return 0;            // m1 <= m2
+  if (!(chi1 >= 0.0) || !(chi1 <= 1.0) || !(chi2 >= 0.0) || !(chi2 <= 1.0)) return 0;
+  if (!std::isfinite(kq1) || !std::isfinite(kq2)) return 0;
+  return 1;
+}
+
+// ---- evaluation kernel for mc_eval ---------------------------------------------------------------
+template <bool PER_ORBIT, bool QM>
+__global__ void __launch_bounds__(mc::kBlock)
+eval_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ mc::IntegrateArgs A, int what, int mode,
+            const double* __restrict__ refs, double* __restrict__ out) {
+  extern __shared__ double smem[];
+  const int64_t t = (int64_t)blockIdx.x * mc::kBlock + threadIdx.x;
+  const bool active = t < A.n;
+  const int64_t o = active ? t : A.n - 1;
+  using CP = typename std::conditional<PER_ORBIT, mc::SharedConsts, mc::UniformConsts>::type;
+  CP c = [&]() {
+    if constexpr (PER_ORBIT) {
+      mc_derive_consts(A.beta[o], A.chi1[o], A.chi2[o], A.kq1[o], A.kq2[o], A.terms, smem + threadIdx.x, mc::kBlock);
+      return mc::SharedConsts{smem + threadIdx.x, mc::kBlock};
+    } else {
+      return mc::UniformConsts{uc};
+    }
+  }();
+  double z[12], f[12];
+#pragma unroll
+  for (int i = 0; i < 12; ++i) z[i] = A.states[(int64_t)i * A.n + o];
+  int rows = 12;
+  if (what == 0) {
+    f[0] = mc::hamiltonian<QM>(c, z);
+    rows = 1;
+  } else if (what == 1) {
+    mc::pn_rhs<QM>(c, z, f);
+  } else if (what == 2) {
+    mc::six_integrals<QM>(c, z, f);
+    rows = 6;
+  } else if (what == 3) {
+    mc::rk4_step<QM>(c, z, A.h, f);
+  } else {
+    mc::Refs R;
+    R.E0 = refs[o];
+    R.J0[0] = refs[A.n + o]; R.J0[1] = refs[2 * A.n + o]; R.J0[2] = refs[3 * A.n + o];
+    if (mode == 1) mc::correct<1, QM>(c, z, R, A.newton_iters, A.newton_tol);
+    else if (mode == 2) mc::correct<2, QM>(c, z, R, A.newton_iters, A.newton_tol);
+    else if (mode == 3) mc::correct<3, QM>(c, z, R, A.newton_iters, A.newton_tol);
+#pragma unroll
+    for (int i = 0; i < 12; ++i) f[i] = z[i];
+  }
+  if (active) {
+#pragma unroll
+    for (int i = 0; i < 12; ++i)
+      if (i < rows) out[(int64_t)i * A.n + o] = f[i];
+  }
+}
+
+// ---- DFMA throughput probe -------------------------------------------------------------------------
+// 16 independent FMA chains per thread, 256 threads per block, 8 blocks per SM resident.
+__global__ void __launch_bounds__(256)
+dfma_peak_kernel(double* sink, int iters, double a, double b) {
+  double x[16];
+#pragma unroll
+  for (int j = 0; j < 16; ++j) x[j] = 1.0 + 1e-9 * (threadIdx.x + j);
+#pragma unroll 1
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int rep = 0; rep < 8; ++rep) {
+#pragma unroll
+      for (int j = 0; j < 16; ++j) x[j] = fma(x[j], a, b);
+    }
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int j = 0; j < 16; ++j) s += x[j];
+  if (s == 123.456) sink[0] = s;   // never true: keeps the chains alive
+}
+
+void fill_args(const mc_handle* h, mc::IntegrateArgs& A) {
+  memset(&A, 0, sizeof(A));
+  A.beta = h->P.d_beta; A.chi1 = h->P.d_chi1; A.chi2 = h->P.d_chi2; A.kq1 = h->P.d_kq1; A.kq2 = h->P.d_kq2;
+  A.terms = h->P.terms;
+  A.renorm_interval = h->P.renorm_interval;
+  A.newton_iters = h->P.newton_iters;
+  A.newton_tol = h->P.newton_tol;
+  A.r_merge2 = h->P.r_merge * h->P.r_merge;
+  A.r_escape2 = h->P.r_escape * h->P.r_escape;
+}
+
+}  // namespace
+
+extern "C" {
+
+int mc_params_default(mc_params* p) {
+  if (!p) return MC_EINVAL;
+  memset(p, 0, sizeof(*p));
+  p->struct_size = (uint32_t)sizeof(mc_params);
+  p->terms = MC_TERM_1PN | MC_TERM_2PN | MC_TERM_SO | MC_TERM_S1S2;
+  p->device = 0;
+  p->per_orbit = 0;
+  p->beta = p->chi1 = p->chi2 = p->kq1 = p->kq2 = 1.0;
+  p->renorm_interval = 100;
+  p->newton_iters = 2;
+  p->newton_tol = 1e-10;
+  p->r_merge = 2.0;
+  p->r_escape = 1e4;
+  p->cuda_stream = nullptr;
+  return MC_OK;
+}
+
+int mc_create(const mc_params* params, mc_handle** out_handle) {
+  if (!params || !out_handle) return MC_EINVAL;
+  if (params->struct_size != sizeof(mc_params)) return MC_EINVAL;
+  if (params->terms & ~31u) return MC_EINVAL;
+  if (params->renorm_interval <= 0 || params->newton_iters < 1 || params->newton_iters > 16) return MC_EINVAL;
+  if (!(params->newton_tol >= 0.0) || !(params->r_merge >= 0.0) || !(params->r_escape > params->r_merge)) return MC_EINVAL;
+  if (params->per_orbit) {
+    if (!params->d_beta || !params->d_chi1 || !params->d_chi2 || !params->d_kq1 || !params->d_kq2) return MC_EINVAL;
+  } else if (!valid_scalars(params->beta, params->chi1, params->chi2, params->kq1, params->kq2)) {
+    return MC_EINVAL;
+  }
+  int ndev = 0;
+  MC_CUDA(cudaGetDeviceCount(&ndev));
+  if (params->device < 0 || params->device >= ndev) return MC_EINVAL;
+  cudaDeviceProp prop;
+  MC_CUDA(cudaGetDeviceProperties(&prop, params->device));
+  if (prop.major != 10) return MC_EARCH;   // the fat binary holds sm_100a SASS only
+  MC_CUDA(cudaSetDevice(params->device));
+  mc_handle* h = new (std::nothrow) mc_handle();
+  if (!h) return MC_ENOMEM;
+  h->P = *params;
+  h->stream = (cudaStream_t)params->cuda_stream;
+  h->num_sms = prop.multiProcessorCount;
+  h->last_n = 0;
+  memset(&h->info, 0, sizeof(h->info));
+  if (params->per_orbit) memset(&h->uc, 0, sizeof(h->uc));
+  else mc_derive_consts(params->beta, params->chi1, params->chi2, params->kq1, params->kq2, params->terms, h->uc.v);
+  *out_handle = h;
+  return MC_OK;
+}
+
+int mc_integrate(mc_handle* h, const double* states, int64_t n_orbits, double step_h, int64_t n_steps,
+                 int32_t correction_mode, double shadow_eps, double* out_states, double* out_invariants,
+                 double* out_fli) {
+  if (!h || n_orbits < 0 || n_steps < 0) return MC_EINVAL;
+  if (correction_mode < 0 || correction_mode > 3) return MC_EINVAL;
+  if (!std::isfinite(step_h) || !std::isfinite(shadow_eps)) return MC_EINVAL;
+  const bool shadow = shadow_eps != 0.0;
+  if (n_orbits > 0 && (!states || !out_states || (shadow && !out_fli))) return MC_EINVAL;
+  if (n_orbits > (int64_t)1 << 40) return MC_EINVAL;
+  MC_CUDA(cudaSetDevice(h->P.device));
+  h->last_n = n_orbits;
+  if (n_orbits == 0) return MC_OK;
+  int rc = h->status.reserve(sizeof(int32_t) * (size_t)n_orbits);
+  if (rc) return rc;
+  rc = h->step.reserve(sizeof(int64_t) * (size_t)n_orbits);
+  if (rc) return rc;
+
+  mc::IntegrateArgs A;
+  fill_args(h, A);
+  A.states = states; A.out_states = out_states; A.out_inv = out_invariants; A.out_fli = shadow ? out_fli : nullptr;
+  A.out_status = (int32_t*)h->status.p; A.out_step = (int64_t*)h->step.p;
+  A.n = n_orbits; A.n_steps = n_steps; A.h = step_h; A.shadow_eps = shadow_eps;
+
+  const bool qm = (h->P.terms & MC_TERM_QM) != 0;
+  mc::LaunchFn fn = nullptr;
+  switch (correction_mode) {
+    case 0: fn = mc::launcher_mode0(h->P.per_orbit != 0, qm); break;
+    case 1: fn = mc::launcher_mode1(h->P.per_orbit != 0, qm); break;
+    case 2: fn = mc::launcher_mode2(h->P.per_orbit != 0, qm); break;
+    default: fn = mc::launcher_mode3(h->P.per_orbit != 0, qm); break;
+  }
+  const int64_t traj = n_orbits * (shadow ? 2 : 1);
+  const int64_t grid = (traj + mc::kBlock - 1) / mc::kBlock;
+  if (grid > 0x7fffffffLL) return MC_EINVAL;
+  mc::KernelInfo ki;
+  MC_CUDA(fn(h->uc, A, (int)grid, h->stream, &ki));
+  h->info.grid = (int32_t)grid;
+  h->info.block = ki.block;
+  h->info.regs_per_thread = ki.regs;
+  h->info.local_bytes = ki.local_bytes;
+  h->info.blocks_per_sm = ki.blocks_per_sm;
+  h->info.num_sms = h->num_sms;
+  h->info.smem_bytes = (int32_t)ki.smem;
+  h->info.variant = (h->P.per_orbit ? 1 : 0) | (qm ? 2 : 0) | (correction_mode << 4);
+  h->info.trajectories = traj;
+  return MC_OK;
+}
+
+int mc_get_status(mc_handle* h, int32_t* out_status, int64_t* out_step) {
+  if (!h) return MC_EINVAL;
+  if (h->last_n == 0) return MC_OK;
+  MC_CUDA(cudaSetDevice(h->P.device));
+  if (out_status)
+    MC_CUDA(cudaMemcpyAsync(out_status, h->status.p, sizeof(int32_t) * (size_t)h->last_n, cudaMemcpyDeviceToDevice, h->stream));
+  if (out_step)
+    MC_CUDA(cudaMemcpyAsync(out_step, h->step.p, sizeof(int64_t) * (size_t)h->last_n, cudaMemcpyDeviceToDevice, h->stream));
+  return MC_OK;
+}
+
+int mc_integrate_host(mc_handle* h, const double* states, int64_t n_orbits, double step_h, int64_t n_steps,
+                      int32_t correction_mode, double shadow_eps, double* out_states, double* out_invariants,
+                      double* out_fli, int32_t* out_status, int64_t* out_step) {
+  if (!h || n_orbits < 0) return MC_EINVAL;
+  const bool shadow = shadow_eps != 0.0;
+  if (n_orbits > 0 && (!states || !out_states || (shadow && !out_fli))) return MC_EINVAL;
+  if (n_orbits == 0) { h->last_n = 0; return MC_OK; }
+  MC_CUDA(cudaSetDevice(h->P.device));
+  const size_t sb = sizeof(double) * 12 * (size_t)n_orbits;
+  int rc;
+  if ((rc = h->h_in.reserve(sb))) return rc;
+  if ((rc = h->h_out.reserve(sb))) return rc;
+  if (out_invariants && (rc = h->h_inv.reserve(sb))) return rc;
+  if (shadow && (rc = h->h_fli.reserve(sizeof(double) * (size_t)n_orbits))) return rc;
+  MC_CUDA(cudaMemcpyAsync(h->h_in.p, states, sb, cudaMemcpyHostToDevice, h->stream));
+  rc = mc_integrate(h, (const double*)h->h_in.p, n_orbits, step_h, n_steps, correction_mode, shadow_eps,
+                    (double*)h->h_out.p, out_invariants ? (double*)h->h_inv.p : nullptr,
+                    shadow ? (double*)h->h_fli.p : nullptr);
+  if (rc) return rc;
+  MC_CUDA(cudaMemcpyAsync(out_states, h->h_out.p, sb, cudaMemcpyDeviceToHost, h->stream));
+  if (out_invariants) MC_CUDA(cudaMemcpyAsync(out_invariants, h->h_inv.p, sb, cudaMemcpyDeviceToHost, h->stream));
+  if (shadow) MC_CUDA(cudaMemcpyAsync(out_fli, h->h_fli.p, sizeof(double) * (size_t)n_orbits, cudaMemcpyDeviceToHost, h->stream));
+  if (out_status) MC_CUDA(cudaMemcpyAsync(out_status, h->status.p, sizeof(int32_t) * (size_t)n_orbits, cudaMemcpyDeviceToHost, h->stream));
+  if (out_step) MC_CUDA(cudaMemcpyAsync(out_step, h->step.p, sizeof(int64_t) * (size_t)n_orbits, cudaMemcpyDeviceToHost, h->stream));
+  MC_CUDA(cudaStreamSynchronize(h->stream));
+  return MC_OK;
+}
+
+int mc_eval(mc_handle* h, int32_t what, const double* states, int64_t n, double step_h, int32_t mode,
+            const double* refs, double* out) {
+  if (!h || n < 0 || what < 0 || what > 4) return MC_EINVAL;
+  if (n == 0) return MC_OK;
+  if (!states || !out) return MC_EINVAL;
+  if (what == 4 && (mode < 0 || mode > 3 || (mode >= 2 && !refs))) return MC_EINVAL;
+  MC_CUDA(cudaSetDevice(h->P.device));
+  mc::IntegrateArgs A;
+  fill_args(h, A);
+  A.states = states; A.n = n; A.h = step_h;
+  const bool qm = (h->P.terms & MC_TERM_QM) != 0, po = h->P.per_orbit != 0;
+  const int grid = (int)((n + mc::kBlock - 1) / mc::kBlock);
+  const size_t smem = po ? sizeof(double) * MC_NCONST * mc::kBlock : 0;
+  if (po && qm) eval_kernel<true, true><<<grid, mc::kBlock, smem, h->stream>>>(h->uc, A, what, mode, refs, out);
+  else if (po) eval_kernel<true, false><<<grid, mc::kBlock, smem, h->stream>>>(h->uc, A, what, mode, refs, out);
+  else if (qm) eval_kernel<false, true><<<grid, mc::kBlock, smem, h->stream>>>(h->uc, A, what, mode, refs, out);
+  else eval_kernel<false, false><<<grid, mc::kBlock, smem, h->stream>>>(h->uc, A, what, mode, refs, out);
+  MC_CUDA(cudaGetLastError());
+  return MC_OK;
+}
+
+int mc_last_launch_info(mc_handle* h, mc_launch_info* out) {
+  if (!h || !out) return MC_EINVAL;
+  *out = h->info;
+  return MC_OK;
+}
+
+int mc_fp64_peak(int32_t device, double millis, double* out_tflops, double* out_sm_clock_mhz) {
+  if (!out_tflops || !(millis > 0.0)) return MC_EINVAL;
+  MC_CUDA(cudaSetDevice(device));
+  cudaDeviceProp prop;
+  MC_CUDA(cudaGetDeviceProperties(&prop, device));
+  double* sink = nullptr;
+  MC_CUDA(cudaMalloc(&sink, sizeof(double)));
+  cudaEvent_t e0, e1;
+  MC_CUDA(cudaEventCreate(&e0));
+  MC_CUDA(cudaEventCreate(&e1));
+  const int grid = prop.multiProcessorCount * 8, block = 256;
+  int iters = 2000;
+  double best = 0.0;
+  float ms = 0.f;
+  for (int pass = 0; pass < 6; ++pass) {
+    MC_CUDA(cudaEventRecord(e0, 0));
+    dfma_peak_kernel<<<grid, block>>>(sink, iters, 0.999999999, 1e-9);
+    MC_CUDA(cudaEventRecord(e1, 0));
+    MC_CUDA(cudaEventSynchronize(e1));
+    MC_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    const double flops = 2.0 * 16.0 * 8.0 * (double)iters * (double)grid * block;
+    const double tf = flops / (ms * 1e-3) / 1e12;
+    if (pass >= 2 && tf > best) best = tf;               // passes 0-1 size the run and warm the clocks
+    if (pass < 2 && ms > 0.f) iters = (int)fmin(2.0e6, fmax(100.0, iters * millis / ms));
+  }
+  *out_tflops = best;
+  if (out_sm_clock_mhz) {
+    // cycles per second implied by one DFMA per lane per clock on 64 lanes per SM
+    *out_sm_clock_mhz = best * 1e12 / (2.0 * 64.0 * prop.multiProcessorCount) / 1e6;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(sink);
+  return MC_OK;
+}
+
+int mc_destroy(mc_handle* h) {
+  if (!h) return MC_EINVAL;
+  cudaSetDevice(h->P.device);
+  h->status.release(); h->step.release();
+  h->h_in.release(); h->h_out.release(); h->h_inv.release(); h->h_fli.release();
+  delete h;
+  return MC_OK;
+}
+
+const char* mc_strerror(int code) {
+  switch (code) {
+    case MC_OK: return "ok";
+    case MC_EINVAL: return "invalid argument";
+    case MC_ECUDA: return g_cuda_msg;
+    case MC_EARCH: return "device is not compute capability 10.x (library holds sm_100a code only)";
+    case MC_ENOMEM: return "host allocation failed";
+    default: return "unknown mc_error";
+  }
+}
+
+}  // extern "C"

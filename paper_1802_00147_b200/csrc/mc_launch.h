@@ -1,0 +1,16 @@
+// mc_launch.h -- host-side table of the integrate_kernel instantiations (one .cu per correction mode
+// so the heavy kernels compile in parallel).
+#pragma once
+#include <cuda_runtime.h>
+
+#include "mc_consts.h"
+
+namespace mc {
+struct IntegrateArgs;
+struct KernelInfo { int regs, local_bytes, blocks_per_sm, block; size_t smem; };
+typedef cudaError_t (*LaunchFn)(const McConsts&, const IntegrateArgs&, int grid, cudaStream_t, KernelInfo*);
+LaunchFn launcher_mode0(bool per_orbit, bool qm);
+LaunchFn launcher_mode1(bool per_orbit, bool qm);
+LaunchFn launcher_mode2(bool per_orbit, bool qm);
+LaunchFn launcher_mode3(bool per_orbit, bool qm);
+}  // namespace mc

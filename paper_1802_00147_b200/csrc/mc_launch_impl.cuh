@@ -1,0 +1,45 @@
+// mc_launch_impl.cuh -- included by mc_kernel_mode<N>.cu with MC_MODE defined.
+#pragma once
+#include <type_traits>
+
+#include "mc_kernel.cuh"
+#include "mc_launch.h"
+
+namespace mc {
+
+// Resident 128-thread blocks per SM the register allocator must allow.  Uniform parameters are
+// constant-bank operands, so 3 blocks (<= 168 registers) fit without spills; per-orbit parameters need
+// <= 255 registers (2 blocks).  ptxas -v: 0 spill bytes for all 16 instantiations (profiles/).
+#ifndef MC_MINB_UNIFORM
+#define MC_MINB_UNIFORM 3
+#endif
+#ifndef MC_MINB_PER_ORBIT
+#define MC_MINB_PER_ORBIT 2
+#endif
+
+template <bool PER_ORBIT, bool QM, int MODE>
+static cudaError_t launch(const McConsts& uc, const IntegrateArgs& A, int grid, cudaStream_t stream, KernelInfo* info) {
+  auto kern = integrate_kernel<PER_ORBIT, QM, MODE, (PER_ORBIT ? MC_MINB_PER_ORBIT : MC_MINB_UNIFORM)>;
+  const size_t smem = PER_ORBIT ? sizeof(double) * MC_NCONST * kBlock : 0;
+  if (info) {
+    cudaFuncAttributes fa;
+    cudaError_t e = cudaFuncGetAttributes(&fa, kern);
+    if (e != cudaSuccess) return e;
+    info->regs = fa.numRegs;
+    info->local_bytes = (int)fa.localSizeBytes;
+    info->block = kBlock;
+    info->smem = smem;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&info->blocks_per_sm, kern, kBlock, smem);
+    if (e != cudaSuccess) return e;
+  }
+  if (grid > 0) kern<<<grid, kBlock, smem, stream>>>(uc, A);
+  return cudaGetLastError();
+}
+
+template <int MODE>
+static LaunchFn pick(bool per_orbit, bool qm) {
+  if (per_orbit) return qm ? launch<true, true, MODE> : launch<true, false, MODE>;
+  return qm ? launch<false, true, MODE> : launch<false, false, MODE>;
+}
+
+}  // namespace mc

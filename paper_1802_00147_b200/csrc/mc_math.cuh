@@ -1,0 +1,203 @@
+// mc_math.cuh -- per-trajectory device math: fused Hamiltonian / gradient / precession routine,
+// classical RK4, correction operators.  Everything lives in registers; one thread = one trajectory.
+//
+// Formulation: unit spins, raw dot products (no unit vector n), all inverse
+// powers of r from one rsqrt, Horner polynomials in P = p.p, Q = (n.p)^2, u = 1/r, FMA-first.
+// The oracle (oracle/pn_oracle.hpp) is written differently on purpose; the two share no code.
+#pragma once
+#include "mc_consts.h"
+
+namespace mc {
+
+// ---- constant providers -------------------------------------------------------------------------
+// Uniform parameters: the struct is a __grid_constant__ kernel parameter, so c[i] is a constant-bank
+// operand of the DFMA itself (no register, no load).  Per-orbit parameters: one slot per thread in
+// shared memory, laid out [MC_NCONST][blockDim.x] (conflict-free LDS.64).
+struct UniformConsts {
+  const McConsts& k;
+  __device__ __forceinline__ double operator[](int i) const { return k.v[i]; }
+};
+struct SharedConsts {
+  const double* base;  // &smem[threadIdx.x]
+  int stride;          // blockDim.x
+  __device__ __forceinline__ double operator[](int i) const { return base[i * stride]; }
+};
+
+// ---- small helpers ------------------------------------------------------------------------------
+__device__ __forceinline__ double dot3(const double* a, const double* b) {
+  return fma(a[2], b[2], fma(a[1], b[1], a[0] * b[0]));
+}
+// c = a x b
+__device__ __forceinline__ void cross3(const double* a, const double* b, double* c) {
+  c[0] = fma(a[1], b[2], -(a[2] * b[1]));
+  c[1] = fma(a[2], b[0], -(a[0] * b[2]));
+  c[2] = fma(a[0], b[1], -(a[1] * b[0]));
+}
+
+// 1/sqrt(x) for x > 0, normal: MUFU.RSQ64H seed (~2^-22 relative) + one third-order step
+// y <- y (1 + e/2 + 3 e^2/8), e = 1 - x y^2  => relative error ~ 1e-20 before rounding.
+__device__ __forceinline__ double rsqrt_pos(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double e = fma(-x, y * y, 1.0);
+  const double q = fma(0.375, e, 0.5) * e;
+  return fma(y, q, y);
+}
+
+// 1/x for finite normal x != 0: MUFU.RCP64H seed + two Newton steps.
+__device__ __forceinline__ double rcp_nz(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = fma(-x, y, 1.0);
+  y = fma(y, fma(e, e, e), y);   // y (1 + e + e^2): error e^3
+  e = fma(-x, y, 1.0);
+  return fma(y, e, y);
+}
+
+__device__ __forceinline__ bool finite12(const double* z) {
+  // exponent field all ones <=> inf or nan; integer pipe only (keeps the FP64 pipe for the physics)
+  unsigned bad = 0;
+#pragma unroll
+  for (int i = 0; i < 12; ++i) bad |= ((unsigned)__double2hiint(z[i]) & 0x7ff00000u) == 0x7ff00000u;
+  return bad == 0;
+}
+
+// ---- the fused model routine ----------------------------------------------------------------------
+// Input  z = (r[0:3], p[3:6], sigma1[6:9], sigma2[9:12]).
+// Output g[0:3] = dH/dr, g[3:6] = dH/dp; if OMEGA: g[6:9] = Omega1, g[9:12] = Omega2; if WANT_H: H.
+// eqs (1)-(9) of the paper with the readings of DESIGN.md section 3.
+template <bool QM, bool OMEGA, bool WANT_H, class C>
+__device__ __forceinline__ void pn_eval(const C& c, const double* z, double* g, double& H) {
+  const double* r = z;
+  const double* p = z + 3;
+  const double* s1 = z + 6;
+  const double* s2 = z + 9;
+  const double r2 = dot3(r, r);
+  const double u = rsqrt_pos(r2);
+  const double u2 = u * u, u3 = u2 * u, u5 = u3 * u2;
+  const double rp = dot3(r, p);
+  const double P = dot3(p, p);
+  const double npu = rp * u;
+  const double Q = npu * npu;
+
+  // orbital polynomials (Horner)
+  const double t1 = fma(c[K_D2], Q, fma(c[K_D1], P, c[K_B1]));   // b1 + d1 P + d2 Q
+  const double t2 = fma(c[K_D3], Q, c[K_B2]);                    // b2 + d3 Q
+  const double t3 = fma(c[K_E2], Q, c[K_E1] * P);                // e1 P + e2 Q
+  // H_P = 1/2 + P (2 a1 + 3 c3 P) + u (b1 + 2 d1 P + d2 Q + e1 u)
+  const double hp_u = fma(c[K_E1], u, fma(c[K_D1], P, t1));
+  const double HP = fma(u, hp_u, fma(P, fma(3.0 * c[K_C3], P, 2.0 * c[K_A1]), 0.5));
+  // H_Q = u (b2 + d2 P + 2 d3 Q + e2 u)
+  const double HQ = u * fma(c[K_E2], u, fma(c[K_D2], P, fma(c[K_D3], Q, t2)));
+  // H_u = -1 + P t1 + Q t2 + u (2 h1 + 2 t3 + 3 f1 u)
+  const double hu_u = fma(3.0 * c[K_F1], u, fma(2.0, t3, 2.0 * c[K_H1]));
+  const double Hu = fma(u, hu_u, fma(Q, t2, fma(P, t1, -1.0)));
+  const double A = HP + HP;                                // dH_orb/dp = A p + B r
+  const double B = (HQ + HQ) * (rp * u2);                  // dH_orb/dr = B p + Cc r
+  const double Cc = -u2 * fma(Hu, u, (HQ + HQ) * Q);
+
+  // spin couplings
+  const double a1 = dot3(s1, r), a2 = dot3(s2, r), d12 = dot3(s1, s2);
+  const double k1u = c[K_K1] * u3, k2u = c[K_K2] * u3;
+  double Sg[3], L[3], SxR[3], PxS[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) Sg[i] = fma(k2u, s2[i], k1u * s1[i]);   // u^3 (k1 sigma1 + k2 sigma2)
+  cross3(r, p, L);
+  cross3(Sg, r, SxR);
+  cross3(p, Sg, PxS);
+  const double LS = dot3(L, Sg);                                      // = H_SO
+  const double a12u5 = a1 * a2 * u5;
+  const double c12u3 = c[K_C12] * u3;
+  // coefficient of r in dH_spin/dr, in units of u^2:  -3 H_SO + c12 (3 d12 u^3 - 15 a1 a2 u^5) + QM
+  double wr = fma(c12u3, 3.0 * d12, fma(-15.0 * c[K_C12], a12u5, -3.0 * LS));
+  const double c12u5x3 = 3.0 * c[K_C12] * u5;
+  double w1 = c12u5x3 * a2, w2 = c12u5x3 * a1;
+  double Hss = fma(3.0 * c[K_C12], a12u5, -(c12u3 * d12));
+  if (QM) {
+    const double d11 = dot3(s1, s1), d22 = dot3(s2, s2);
+    const double q1u3 = c[K_Q1] * u3, q2u3 = c[K_Q2] * u3;
+    const double a11u5 = a1 * a1 * u5, a22u5 = a2 * a2 * u5;
+    wr = fma(q1u3, 3.0 * d11, fma(-15.0 * c[K_Q1], a11u5, wr));
+    wr = fma(q2u3, 3.0 * d22, fma(-15.0 * c[K_Q2], a22u5, wr));
+    w1 = fma(6.0 * c[K_Q1] * u5, a1, w1);
+    w2 = fma(6.0 * c[K_Q2] * u5, a2, w2);
+    Hss += fma(3.0 * c[K_Q1], a11u5, -(q1u3 * d11)) + fma(3.0 * c[K_Q2], a22u5, -(q2u3 * d22));
+  }
+  const double Cr = fma(wr, u2, Cc);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    g[i] = fma(w2, s2[i], fma(w1, s1[i], fma(Cr, r[i], fma(B, p[i], PxS[i]))));
+    g[3 + i] = fma(A, p[i], fma(B, r[i], SxR[i]));
+  }
+  if (OMEGA) {
+    const double o1u = c[K_O1] * u3, o2u = c[K_O2] * u3;
+    const double m12u = c[K_M12] * u3, m21u = c[K_M21] * u3;
+    double b1r = c[K_M12] * a2, b2r = c[K_M21] * a1;
+    if (QM) { b1r = fma(c[K_M11], a1, b1r); b2r = fma(c[K_M22], a2, b2r); }
+    b1r *= 3.0 * u5;
+    b2r *= 3.0 * u5;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      g[6 + i] = fma(-m12u, s2[i], fma(b1r, r[i], o1u * L[i]));
+      g[9 + i] = fma(-m21u, s1[i], fma(b2r, r[i], o2u * L[i]));
+    }
+  }
+  if (WANT_H) {
+    // H = P/2 - u + P^2 (a1 + c3 P) + u (P t1 + Q t2) + u^2 (h1 + t3) + f1 u^3 + H_SO + H_SS
+    const double orb = fma(u2, fma(c[K_F1], u, c[K_H1] + t3), fma(u, fma(Q, t2, P * t1), fma(P * P, fma(c[K_C3], P, c[K_A1]), fma(0.5, P, -u))));
+    H = orb + (LS + Hss);
+  }
+}
+
+// dz/dt, eqs (6)-(7): dr/dt = dH/dp, dp/dt = -dH/dr, dsigma_i/dt = Omega_i x sigma_i.
+template <bool QM, class C>
+__device__ __forceinline__ void pn_rhs(const C& c, const double* z, double* f) {
+  double g[12], H;
+  pn_eval<QM, true, false>(c, z, g, H);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { f[i] = g[3 + i]; f[3 + i] = -g[i]; }
+  cross3(g + 6, z + 6, f + 6);
+  cross3(g + 9, z + 9, f + 9);
+}
+
+// J = r x p + s1 sigma1 + s2 sigma2
+template <class C>
+__device__ __forceinline__ void total_J(const C& c, const double* z, double* J) {
+  cross3(z, z + 3, J);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) J[i] = fma(c[K_S2], z[9 + i], fma(c[K_S1], z[6 + i], J[i]));
+}
+
+template <bool QM, class C>
+__device__ __forceinline__ double hamiltonian(const C& c, const double* z) {
+  double g[12], H;
+  pn_eval<QM, false, true>(c, z, g, H);
+  return H;
+}
+
+// Classical RK4 (R9), low-storage bookkeeping: y (kept), acc, stage input yt.
+template <bool QM, class C>
+__device__ __forceinline__ void rk4_step(const C& c, const double* y, double h, double* out) {
+  const double h2 = 0.5 * h, h3 = h * (1.0 / 3.0), h6 = h * (1.0 / 6.0);
+  double k[12], yt[12];
+  pn_rhs<QM>(c, y, k);
+#pragma unroll
+  for (int i = 0; i < 12; ++i) { out[i] = fma(h6, k[i], y[i]); yt[i] = fma(h2, k[i], y[i]); }
+  pn_rhs<QM>(c, yt, k);
+#pragma unroll
+  for (int i = 0; i < 12; ++i) { out[i] = fma(h3, k[i], out[i]); yt[i] = fma(h2, k[i], y[i]); }
+  pn_rhs<QM>(c, yt, k);
+#pragma unroll
+  for (int i = 0; i < 12; ++i) { out[i] = fma(h3, k[i], out[i]); yt[i] = fma(h, k[i], y[i]); }
+  pn_rhs<QM>(c, yt, k);
+#pragma unroll
+  for (int i = 0; i < 12; ++i) out[i] = fma(h6, k[i], out[i]);
+}
+
+// eq (10): sigma <- sigma / |sigma|
+__device__ __forceinline__ void normalise3(double* s) {
+  const double w = rsqrt_pos(dot3(s, s));
+  s[0] *= w; s[1] *= w; s[2] *= w;
+}
+
+}  // namespace mc

@@ -1,0 +1,295 @@
+"""GPU parity: libmc (through the C ABI, paper_1802_00147_b200.binding) vs the CPU oracle, element by
+element on the same seeded inputs.  Tolerances (DESIGN.md section 7 / BASELINE.json north_star):
+state relative error <= 1e-10 after 1e3 steps; six integrals' relative drift <= 1e-12 with correction
+on; FLI class agreement; integer outputs (status, steps) exact."""
+import numpy as np
+import pytest
+
+import oracle
+from conftest import random_states
+from paper_1802_00147_b200 import workloads
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+STATE_RTOL = 1e-10      # north_star
+DRIFT_TOL = 1e-12       # north_star
+FLI_THRESHOLD = 5.8
+
+
+@pytest.fixture(scope="module")
+def mc():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1802_00147_b200 import binding
+    return binding
+
+
+def rel_state_err(a, b):
+    """max over orbits of per-block relative error (r, p, S1, S2 blocks)."""
+    worst = 0.0
+    for s in (slice(0, 3), slice(3, 6), slice(6, 9), slice(9, 12)):
+        num = np.linalg.norm(a[s] - b[s], axis=0)
+        den = np.linalg.norm(b[s], axis=0)
+        worst = max(worst, float((num / den).max()))
+    return worst
+
+
+def drift(states, inv0, **params):
+    """Relative drift of the six integrals, evaluated by the ORACLE (long double) on given states."""
+    I1 = oracle.integrals(states, **params)
+    dE = np.abs(I1[0] - inv0[0]) / np.abs(inv0[0])
+    dJ = np.linalg.norm(I1[1:4] - inv0[1:4], axis=0) / np.linalg.norm(inv0[1:4], axis=0)
+    return max(dE.max(), dJ.max(), np.abs(I1[4] - 1).max(), np.abs(I1[5] - 1).max())
+
+
+PARAM_SETS = [
+    dict(beta=1.0, chi1=1.0, chi2=1.0, kq1=1.0, kq2=1.0),
+    dict(beta=0.8, chi1=0.9, chi2=0.9, kq1=3.0, kq2=5.5),
+    dict(beta=1.0 / 3.0, chi1=0.75, chi2=0.75, kq1=1.0, kq2=1.0),
+]
+
+
+@pytest.mark.parametrize("terms", [0, 1, 3, 4, 8, 15, 16, 31])
+@pytest.mark.parametrize("pset", [0, 1, 2])
+def test_model_routines_match_oracle_uniform(mc, terms, pset):
+    """H, dz/dt, six integrals, one RK4 step: 300 random states (3 blocks, ragged tail)."""
+    z = random_states(300, seed=1000 + terms)
+    par = PARAM_SETS[pset]
+    with mc.Integrator(terms=terms, **par) as I:
+        for what, ofn, scale_rows in (("H", lambda: oracle.hamiltonian(z, terms=terms, **par)[None], None),
+                                      ("rhs", lambda: oracle.rhs(z, terms=terms, **par), 3),
+                                      ("integrals", lambda: oracle.integrals(z, terms=terms, **par), None),
+                                      ("rk4_step", lambda: oracle.rk4_step(z, 1.0, terms=terms, **par), 3)):
+            got = I.eval(what, z, h=1.0).cpu().numpy()
+            want = ofn()
+            if scale_rows:
+                assert rel_state_err_blocks(got, want) < 2e-13, what
+            else:
+                assert np.abs(got - want).max() <= 4e-14 * max(1.0, np.abs(want).max()), what
+
+
+def rel_state_err_blocks(a, b):
+    worst = 0.0
+    for s in (slice(0, 3), slice(3, 6), slice(6, 9), slice(9, 12)):
+        den = np.linalg.norm(b[s], axis=0)
+        num = np.linalg.norm(a[s] - b[s], axis=0)
+        ok = den > 0
+        if ok.any():
+            worst = max(worst, float((num[ok] / den[ok]).max()))
+        assert np.all(num[~ok] == 0)
+    return worst
+
+
+def test_model_routines_match_oracle_per_orbit(mc):
+    z = random_states(257, seed=77)
+    rng = np.random.default_rng(78)
+    par = dict(beta=rng.uniform(0.3, 1, 257), chi1=rng.uniform(0, 1, 257), chi2=rng.uniform(0, 1, 257),
+               kq1=rng.uniform(1, 8, 257), kq2=rng.uniform(1, 8, 257))
+    for terms in (15, 31):
+        with mc.Integrator(terms=terms, **par) as I:
+            assert rel_state_err_blocks(I.eval("rhs", z).cpu().numpy(), oracle.rhs(z, terms=terms, **par)) < 2e-13
+            H = I.eval("H", z).cpu().numpy()[0]
+            assert np.abs(H - oracle.hamiltonian(z, terms=terms, **par)).max() < 1e-15
+
+
+@pytest.mark.parametrize("mode", [1, 2, 3])
+@pytest.mark.parametrize("terms", [15, 31])
+def test_correction_operator_matches_oracle(mc, mode, terms):
+    w = workloads.config0(200)
+    par = dict(beta=0.7, chi1=0.9, chi2=0.8, kq1=2.0, kq2=3.0)
+    I0 = oracle.integrals(w.states, terms=terms, **par)
+    rng = np.random.default_rng(3)
+    zp = w.states * (1 + 1e-7 * rng.normal(size=w.states.shape))
+    want, ok = oracle.correct(zp, I0[0], I0[1:4], mode, terms=terms, newton_iters=4, **par)
+    with mc.Integrator(terms=terms, newton_iters=4, **par) as I:
+        got = I.eval("correct", zp, mode=mode, refs=I0[0:4]).cpu().numpy()
+    assert ok.all()
+    assert rel_state_err(got, want) < 1e-13
+    assert drift(got, I0, terms=terms, **par) < (1e-14 if mode == 3 else 1.0)
+
+
+def test_config0_state_parity_after_1e3_steps_and_drift_after_1e4(mc):
+    """BASELINE config 0: 64 orbits, mode 3, no shadow."""
+    w = workloads.config0()
+    with mc.Integrator(terms=w.terms, beta=1.0, chi1=1.0, chi2=1.0) as I:
+        g3 = I.integrate(w.states, w.h, 1000, 3)
+        g4 = I.integrate(w.states, w.h, 10_000, 3)
+        info = I.launch_info()
+    o3 = oracle.integrate(w.states, w.h, 1000, 3, **w.params())
+    assert rel_state_err(g3.states.cpu().numpy(), o3.states) <= STATE_RTOL
+    assert np.array_equal(g3.status.cpu().numpy(), o3.status)
+    assert np.array_equal(g3.steps_done.cpu().numpy(), o3.steps_done)
+    inv = g4.invariants.cpu().numpy()
+    assert np.abs(inv[0:6] - o3.invariants[0:6]).max() < 1e-14          # reference integrals agree
+    assert drift(g4.states.cpu().numpy(), o3.invariants[0:6], **w.params()) <= DRIFT_TOL
+    assert (g4.status.cpu().numpy() == 0).all()
+    assert info["local_bytes"] == 0                                      # zero register spills
+
+
+@pytest.mark.parametrize("mode", [3, 0])
+def test_config1_shadow_fli_parity_per_orbit_params(mc, mode):
+    """BASELINE config 1 (per-orbit beta, chi; shadow 1e-8, renorm 100), first 150 orbits = 300
+    trajectories: two full blocks + ragged tail; 2000 steps = 20 renormalisations."""
+    w = workloads.config1().subset(np.arange(150))
+    with mc.Integrator(terms=w.terms, **{k: v for k, v in w.params().items() if k != "terms"}) as I:
+        g = I.integrate(w.states, w.h, 2000, mode, shadow_eps=w.shadow_eps)
+    o = oracle.integrate(w.states, w.h, 2000, mode, shadow_eps=w.shadow_eps, **w.params())
+    assert rel_state_err(g.states.cpu().numpy(), o.states) <= 4 * STATE_RTOL   # 2e3 steps
+    assert np.abs(g.fli.cpu().numpy() - o.fli).max() < 1e-3
+    assert np.array_equal(g.status.cpu().numpy(), o.status)
+    assert np.array_equal(g.steps_done.cpu().numpy(), o.steps_done)
+    if mode == 3:
+        assert drift(g.states.cpu().numpy(), o.invariants[0:6], **w.params()) <= DRIFT_TOL
+
+
+def classes(fli, status):
+    """0 regular, 1 chaotic, 2 dropped."""
+    c = (fli >= FLI_THRESHOLD).astype(int)
+    c[(status & 255) != 0] = 2
+    return c
+
+
+def test_scan_grid_with_dropped_orbits_matches_oracle(mc):
+    """Config-2-shaped grid (strong-field corner r0 in [6,16] so that merged orbits occur), 12 x 11
+    cells = 132 orbits, 3000 steps: status, freeze step, FLI and class per cell."""
+    z, R, TH = workloads.scan_grid(12, 11, r_lo=6.0, r_hi=16.0)
+    with mc.Integrator() as I:
+        g = I.integrate(z, 1.0, 3000, 3, shadow_eps=1e-8)
+    o = oracle.integrate(z, 1.0, 3000, 3, shadow_eps=1e-8)
+    gs, gk = g.status.cpu().numpy(), g.steps_done.cpu().numpy()
+    assert (o.status == 1).sum() >= 5 and (o.status == 0).sum() >= 50     # the case has both kinds
+    assert np.array_equal(gs, o.status)
+    assert np.array_equal(gk, o.steps_done)
+    alive = o.status == 0
+    gfli = g.fli.cpu().numpy()
+    assert (classes(gfli, gs) == classes(o.fli, o.status)).mean() >= 0.99
+    calm = alive & (o.fli < 3.5)                       # regular cells: values agree, not only classes
+    assert calm.sum() > 20
+    assert np.abs(gfli[calm] - o.fli[calm]).max() < 1e-2
+    assert rel_state_err(g.states.cpu().numpy()[:, calm], o.states[:, calm]) < 1e-7
+    # frozen cells keep the last good state: |r| >= r_merge
+    assert (np.linalg.norm(g.states.cpu().numpy()[0:3], axis=0) >= 2.0).all()
+
+
+def test_config3_quadrupole_on_off_parity(mc):
+    """BASELINE config 3 subset: beta = 0.8, chi = 0.9, per-orbit kq; QM on vs off on identical inputs."""
+    full = workloads.config3(n_r=16, n_theta=9, qm=True)
+    par = {k: v for k, v in full.params().items() if k != "terms"}
+    out = {}
+    for qm in (True, False):
+        terms = full.terms if qm else (full.terms & ~workloads.TERM_QM)
+        with mc.Integrator(terms=terms, **par) as I:
+            g = I.integrate(full.states, 1.0, 1000, 3, shadow_eps=1e-8)
+        o = oracle.integrate(full.states, 1.0, 1000, 3, shadow_eps=1e-8, terms=terms, **par)
+        ok = o.status == 0
+        assert np.array_equal(g.status.cpu().numpy(), o.status)
+        assert rel_state_err(g.states.cpu().numpy()[:, ok], o.states[:, ok]) <= STATE_RTOL
+        assert np.abs(g.fli.cpu().numpy()[ok] - o.fli[ok]).max() < 1e-3
+        out[qm] = g.states.cpu().numpy()
+    assert np.abs(out[True] - out[False]).max() > 1e-3          # the term really changes the dynamics
+
+
+def test_mode2_dual_scaling_parity_on_unskipped_orbits(mc):
+    w = workloads.config0(128)
+    with mc.Integrator(newton_iters=4) as I:
+        g = I.integrate(w.states, 1.0, 1000, 2)
+    o = oracle.integrate(w.states, 1.0, 1000, 2, newton_iters=4, **w.params())
+    gs = g.status.cpu().numpy()
+    clean = (o.status == 0) & (gs == 0)
+    assert clean.sum() >= 32                                       # singular steps are common (R7)
+    assert ((gs & 256) == (o.status & 256)).mean() > 0.9
+    # The dual-scaling Jacobian is singular where p.dH/dp = r.dH/dr, twice per radial period (R7): steps
+    # near those points amplify rounding differences, so the bound is looser than for mode 3.
+    gz = g.states.cpu().numpy()
+    per_orbit = np.array([rel_state_err(gz[:, [i]], o.states[:, [i]]) for i in np.where(clean)[0]])
+    print("mode-2 per-orbit relative error: median %.2e  p90 %.2e  max %.2e" %
+          (np.median(per_orbit), np.quantile(per_orbit, 0.9), per_orbit.max()))
+    assert np.median(per_orbit) <= 1e-12 and per_orbit.max() <= 1e-8
+    I1 = oracle.integrals(g.states.cpu().numpy()[:, clean], **w.subset(np.where(clean)[0]).params())
+    I0 = o.invariants[0:6, clean]
+    assert np.abs(I1[0] / I0[0] - 1).max() < DRIFT_TOL
+    assert np.abs(np.linalg.norm(I1[1:4], axis=0) / np.linalg.norm(I0[1:4], axis=0) - 1).max() < DRIFT_TOL
+
+
+def test_batch_properties(mc):
+    w = workloads.config0(96)
+    with mc.Integrator() as I:
+        a = I.integrate(w.states, 1.0, 500, 3, shadow_eps=1e-8)
+        perm = np.random.default_rng(0).permutation(96)
+        b = I.integrate(w.states[:, perm], 1.0, 500, 3, shadow_eps=1e-8)
+        same = I.integrate(np.repeat(w.states[:, :1], 70, axis=1), 1.0, 500, 3, shadow_eps=1e-8)
+        A, B = a.states.cpu().numpy(), b.states.cpu().numpy()
+        assert np.array_equal(A[:, perm], B)                                  # orbits are independent
+        assert np.array_equal(a.fli.cpu().numpy()[perm], b.fli.cpu().numpy())
+        S = same.states.cpu().numpy()
+        assert np.array_equal(S, np.repeat(S[:, :1], 70, axis=1))             # lanes are equivalent
+        assert np.array_equal(S[:, 0], A[:, 0])
+        # in-place operation (out_states aliases states)
+        zt = torch.as_tensor(w.states, device="cuda").clone()
+        c = I.integrate(zt, 1.0, 500, 3, shadow_eps=1e-8, out_states=zt)
+        assert np.array_equal(c.states.cpu().numpy(), A)
+        # host-buffer entry point gives the same bits
+        hres = I.integrate_host(w.states, 1.0, 500, 3, shadow_eps=1e-8)
+        assert np.array_equal(hres.states, A) and np.array_equal(hres.fli, a.fli.cpu().numpy())
+        assert np.array_equal(hres.status, a.status.cpu().numpy())
+    with mc.Integrator(terms=31, kq1=0.0, kq2=0.0) as Iq:                      # QM with zero coefficient
+        q = Iq.integrate(w.states, 1.0, 500, 3, shadow_eps=1e-8)
+    assert np.array_equal(q.states.cpu().numpy(), A)
+
+
+def test_edge_cases(mc):
+    w = workloads.config0(129)
+    with mc.Integrator() as I:
+        e = I.integrate(w.states[:, :0], 1.0, 10, 3)
+        assert e.states.shape == (12, 0)
+        one = I.integrate(w.states[:, :1], 1.0, 100, 3, shadow_eps=1e-8)
+        o = oracle.integrate(w.states[:, :1], 1.0, 100, 3, shadow_eps=1e-8)
+        assert rel_state_err(one.states.cpu().numpy(), o.states) < 1e-11
+        zero = I.integrate(w.states, 1.0, 0, 3, shadow_eps=1e-8)                # n_steps = 0
+        assert np.allclose(zero.states.cpu().numpy(), w.states, rtol=1e-15, atol=0)
+        assert np.allclose(zero.fli.cpu().numpy(), 0.0, atol=1e-6)
+        assert (zero.steps_done.cpu().numpy() == 0).all()
+        back = I.integrate(I.integrate(w.states, 1.0, 300, 3).states, -1.0, 300, 3)   # negative step
+        assert rel_state_err(back.states.cpu().numpy(), w.states) < 1e-6
+        bad = w.states[:, :40].copy()
+        bad[1, 7] = np.nan
+        bad[0, 9] = 1.0                                                           # starts inside r_merge... plunges
+        r = I.integrate(bad, 1.0, 50, 3, shadow_eps=1e-8)
+        st = r.status.cpu().numpy()
+        assert st[7] == 3 and r.steps_done.cpu().numpy()[7] == 0
+        assert st[9] in (1, 3)
+        good = np.ones(40, bool)
+        good[[7, 9]] = False
+        assert (st[good] == 0).all()                                              # neighbours are unaffected
+    with pytest.raises(mc.MCError):
+        with mc.Integrator() as I:
+            I.integrate(w.states, 1.0, 10, 7)
+
+
+def test_full_size_scan_sampled_against_oracle(mc):
+    """BASELINE config 2 at full size (314 x 314 orbits, shadow, mode 3) in the launch configuration
+    bench.py times, 1e4 steps here; 48 sampled cells are recomputed one by one by the oracle, and the
+    six-integral drift is checked on every live cell."""
+    w = workloads.config2(n_steps=10_000)
+    with mc.Integrator() as I:
+        g = I.integrate(w.states, w.h, w.n_steps, 3, shadow_eps=w.shadow_eps)
+        info = I.launch_info()
+    assert info["local_bytes"] == 0 and info["trajectories"] == 2 * 314 * 314
+    gs = g.status.cpu().numpy()
+    gz = g.states.cpu().numpy()
+    gfli = g.fli.cpu().numpy()
+    live = gs == 0
+    assert 0.85 < live.mean() < 1.0
+    inv0 = g.invariants.cpu().numpy()[0:6]
+    assert drift(gz[:, live], inv0[:, live], **w.subset(np.where(live)[0]).params()) <= DRIFT_TOL
+    rng = np.random.default_rng(2)
+    idx = np.sort(np.concatenate([rng.choice(314 * 314, 40, replace=False), rng.choice(314 * 40, 8, replace=False)]))
+    sub = w.subset(idx)
+    o = oracle.integrate(sub.states, w.h, w.n_steps, 3, shadow_eps=w.shadow_eps, **sub.params())
+    assert np.array_equal(gs[idx], o.status)
+    assert np.array_equal(g.steps_done.cpu().numpy()[idx], o.steps_done)
+    assert (classes(gfli[idx], gs[idx]) == classes(o.fli, o.status)).mean() >= 0.97
+    reg = (o.status == 0) & (o.fli < 4.0)
+    assert np.abs(gfli[idx][reg] - o.fli[reg]).max() < 0.02
+    assert rel_state_err(gz[:, idx][:, reg], o.states[:, reg]) < 1e-6     # 1e4 steps; regular cells only

@@ -205,7 +205,11 @@ def test_mode2_dual_scaling_parity_on_unskipped_orbits(mc):
     per_orbit = np.array([rel_state_err(gz[:, [i]], o.states[:, [i]]) for i in np.where(clean)[0]])
     print("mode-2 per-orbit relative error: median %.2e  p90 %.2e  max %.2e" %
           (np.median(per_orbit), np.quantile(per_orbit, 0.9), per_orbit.max()))
-    assert np.median(per_orbit) <= 1e-12 and per_orbit.max() <= 1e-8
+    # Bound from the arithmetic ("mode 2"): the oracle's own double instance differs
+    # from its long-double instance by median 1.5e-12 / p90 6.7e-12 / max 4.0e-10 on this very input
+    # (tests/test_oracle_integrator.py::test_mode2_rounding_amplification_sets_the_parity_bound), i.e.
+    # ~10x the mode-3 figure.  The kernel must sit within the same envelope.
+    assert np.median(per_orbit) <= 1e-11 and np.quantile(per_orbit, 0.9) <= 1e-10 and per_orbit.max() <= 1e-8
     I1 = oracle.integrals(g.states.cpu().numpy()[:, clean], **w.subset(np.where(clean)[0]).params())
     I0 = o.invariants[0:6, clean]
     assert np.abs(I1[0] / I0[0] - 1).max() < DRIFT_TOL

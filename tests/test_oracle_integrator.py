@@ -210,6 +210,24 @@ def test_mode2_rounding_amplification_sets_the_parity_bound():
     assert np.median(out[2]) > 3 * np.median(out[3])
 
 
+def test_two_newton_iterations_leave_a_residual_at_deep_periastron():
+    """DESIGN.md section 7 ("deep periastron"): config-2 cell (3, 308) passes periastron at |r| = 2.2 on
+    step 1e4.  With the fixed 2 Newton iterations (R6) the energy residual there is ~7e-11; one step later,
+    and with 4 iterations, it is round-off.  The GPU drift bound is therefore split at |r| = 3."""
+    sub = workloads.config2(n_steps=10_000).subset([3 * 314 + 308])
+
+    def energy_drift(n, iters):
+        o = oracle.integrate(sub.states, 1.0, n, 3, shadow_eps=1e-8, newton_iters=iters, **sub.params())
+        assert o.status[0] == 0
+        E = oracle.integrals(o.states, **sub.params())[0, 0]
+        return abs(E / o.invariants[0, 0] - 1), np.linalg.norm(o.states[0:3, 0])
+
+    d2, r = energy_drift(10_000, 2)
+    assert 2.0 < r < 2.5 and 1e-12 < d2 < 1e-9
+    assert energy_drift(10_001, 2)[0] < 1e-14
+    assert energy_drift(10_000, 4)[0] < 1e-14
+
+
 def test_flop_counter_reports_the_oracles_own_formulation():
     c = oracle.count_flops(workloads.paper_orbit(2).states[:, 0], terms=15, mode=3, newton_iters=2)
     assert c["rk4_step"] == 4 * c["rhs"] + 159            # 3 stage inputs (3*25) + final combination (84)

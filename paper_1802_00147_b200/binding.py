@@ -59,7 +59,8 @@ def load_library():
     if _lib is not None:
         return _lib
     try:
-        path = _build.build()
+        # MC_LIBMC_PATH: use a prebuilt libmc.so (e.g. a box without nvcc) instead of building in-tree
+        path = os.environ.get("MC_LIBMC_PATH") or _build.build()
     except Exception as e:  # nvcc missing or compile error
         if os.path.exists(_build.LIB):
             path = _build.LIB

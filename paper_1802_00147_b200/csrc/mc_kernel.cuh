@@ -31,7 +31,10 @@ struct IntegrateArgs {
 
 enum { ST_OK = 0, ST_MERGED = 1, ST_UNBOUND = 2, ST_NONFINITE = 3, ST_NEWTON_FLAG = 256 };
 
-constexpr int kBlock = 128;
+#ifndef MC_BLOCK
+#define MC_BLOCK 128
+#endif
+constexpr int kBlock = MC_BLOCK;
 
 template <bool QM, class C>
 __device__ __forceinline__ void six_integrals(const C& c, const double* z, double* out6) {
@@ -41,8 +44,16 @@ __device__ __forceinline__ void six_integrals(const C& c, const double* z, doubl
   out6[5] = sqrt(dot3(z + 9, z + 9));
 }
 
+// Register budget: either "MINB resident blocks" (__launch_bounds__) or, with MC_MAXNREG defined, an
+// explicit per-thread cap (__maxnreg__; the two qualifiers exclude each other).
+#ifdef MC_MAXNREG
+#define MC_KERNEL_BOUNDS(MINB) __maxnreg__(MC_MAXNREG)
+#else
+#define MC_KERNEL_BOUNDS(MINB) __launch_bounds__(kBlock, MINB)
+#endif
+
 template <bool PER_ORBIT, bool QM, int MODE, int MINB>
-__global__ void __launch_bounds__(kBlock, MINB)
+__global__ void MC_KERNEL_BOUNDS(MINB)
 integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ IntegrateArgs A) {
   extern __shared__ double smem[];   // PER_ORBIT: [MC_NCONST][kBlock]
   const bool shadow = A.shadow_eps != 0.0;
@@ -67,8 +78,12 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
 #pragma unroll
   for (int i = 0; i < 12; ++i) y[i] = A.states[(int64_t)i * A.n + orbit];
   if (MODE >= 1) { normalise3(y + 6); normalise3(y + 9); }
-  double inv0[6];
-  if (!role_shadow && A.out_inv) six_integrals<QM>(c, y, inv0);   // of the main trajectory, before the offset
+  if (!role_shadow && active && A.out_inv) {   // rows 0-5: the main trajectory before the offset; stored now so
+    double inv0[6];                            // that nothing of it stays in registers during the step loop
+    six_integrals<QM>(c, y, inv0);
+#pragma unroll
+    for (int i = 0; i < 6; ++i) A.out_inv[(int64_t)i * A.n + orbit] = inv0[i];
+  }
   const double d0 = fabs(A.shadow_eps);
   if (role_shadow) y[0] += A.shadow_eps;
   Refs R;
@@ -155,10 +170,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
       double inv1[6];
       six_integrals<QM>(c, y, inv1);
 #pragma unroll
-      for (int i = 0; i < 6; ++i) {
-        A.out_inv[(int64_t)i * A.n + orbit] = inv0[i];
-        A.out_inv[(int64_t)(6 + i) * A.n + orbit] = inv1[i];
-      }
+      for (int i = 0; i < 6; ++i) A.out_inv[(int64_t)(6 + i) * A.n + orbit] = inv1[i];
     }
     A.out_status[orbit] = status | flag;
     A.out_step[orbit] = steps;

@@ -292,7 +292,7 @@ def test_full_size_scan_sampled_against_oracle(mc):
     # periastron"; tests/test_oracle_integrator.py::test_two_newton_iterations_leave_a_residual_at_deep_periastron).
     rfin = np.linalg.norm(gz[0:3], axis=0)
     calm, plunging = live & (rfin >= 3.0), live & (rfin < 3.0)
-    assert plunging.sum() < 0.002 * live.sum()
+    assert plunging.sum() < 0.005 * live.sum()
     assert drift(gz[:, calm], inv0[:, calm], **w.subset(np.where(calm)[0]).params()) <= DRIFT_TOL
     if plunging.any():
         assert drift(gz[:, plunging], inv0[:, plunging], **w.subset(np.where(plunging)[0]).params()) <= 1e-7

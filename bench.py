@@ -20,7 +20,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_1802_00147_b200 import workloads  # noqa: E402
+from paper_1802_00147_b200 import sharding, workloads  # noqa: E402
 
 METRIC = "orbit-RK4-steps/sec (with correction+FLI)"
 UNIT = "orbit-steps/s"
@@ -98,8 +98,7 @@ def global_workload(args, world):
 
 
 def rank_shard(w, args, rank, world):
-    lo, hi = workloads.shard_range(args.grid * world, rank, world)
-    return w.subset(np.arange(lo * args.grid, hi * args.grid))
+    return sharding.rank_shard(w, args.grid, args.grid, rank, world)
 
 
 def cpu_baseline_sample(w, target_seconds=15.0):
@@ -216,10 +215,7 @@ def run_mc(args):
     clocks = sampler.stop()
     kernel_ms = [a.elapsed_time(b) for a, b in ev]
     dev_ms = float(sum(kernel_ms))
-    t = torch.tensor([dev_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    dev_ms_max = float(t.item())
+    dev_ms_max = sharding.max_over_ranks(dev_ms, dev)
     value = orbit_steps_rank * world * args.steps / (dev_ms_max * 1e-3)
 
     # end to end through the C ABI with HOST buffers (pinned): H2D + kernel + D2H inside the timed call
@@ -231,10 +227,7 @@ def run_mc(args):
         hres = I.integrate_host(z_host, w.h, w.n_steps, w.correction_mode, shadow_eps=w.shadow_eps)
     barrier()
     e2e_s = time.perf_counter() - t0
-    t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = orbit_steps_rank * world * args.steps / float(t.item())
+    e2e_value = orbit_steps_rank * world * args.steps / sharding.max_over_ranks(e2e_s, dev)
     h2d = 12 * 8 * n
     d2h = (12 + 12 + 1) * 8 * n + 4 * n + 8 * n
 

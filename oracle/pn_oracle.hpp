@@ -286,9 +286,15 @@ bool dual_scaling(State<T>& z, const Params<T>& P, const Refs<T>& R, int newton_
 // Constraints phi = (H - E0, r x p - Lt); rows of the 4 x 6 Jacobian D are
 // (dH/dr, dH/dp) and, for component k, (p x e_k, e_k x r).  Update
 // (dr, dp) = -D^T (D D^T)^-1 phi.
+// Iteration control as in the paper (R6): Newton
+// steps are repeated until the last update is below the tolerance epsilon,
+// |(dr, dp)|_2 <= newton_tol * |p|_2 (p of the point the step was computed at),
+// at most newton_iters times.  The step that meets the test is still applied.
+// Returns the number of steps taken.
 template <class T>
-void project_six(State<T>& z, const Params<T>& P, const Refs<T>& R, int newton_iters) {
+int project_six(State<T>& z, const Params<T>& P, const Refs<T>& R, int newton_iters, T newton_tol) {
   const V3<T> e[3] = {{T(1), T(0), T(0)}, {T(0), T(1), T(0)}, {T(0), T(0), T(1)}};
+  int done = 0;
   for (int it = 0; it < newton_iters; ++it) {
     const V3<T> Lt = R.J0 - P.s1() * z.s1 - P.s2() * z.s2;
     const Grad<T> G = gradient(z, P);
@@ -300,20 +306,34 @@ void project_six(State<T>& z, const Params<T>& P, const Refs<T>& R, int newton_i
     T A[4][4], lam[4];
     for (int i = 0; i < 4; ++i)
       for (int j = 0; j < 4; ++j) A[i][j] = dot(Dr[i], Dr[j]) + dot(Dp[i], Dp[j]);
-    if (!solve_dense<T, 4>(A, phi, lam)) return;
-    for (int i = 0; i < 4; ++i) { z.r = z.r - lam[i] * Dr[i]; z.p = z.p - lam[i] * Dp[i]; }
+    if (!solve_dense<T, 4>(A, phi, lam)) return done;
+    V3<T> dr = {T(0), T(0), T(0)}, dp = {T(0), T(0), T(0)};
+    for (int i = 0; i < 4; ++i) { dr = dr + lam[i] * Dr[i]; dp = dp + lam[i] * Dp[i]; }
+    const T step2 = dot(dr, dr) + dot(dp, dp);
+    const T scale2 = dot(z.p, z.p);
+    z.r = z.r - dr;
+    z.p = z.p - dp;
+    ++done;
+    if (!(step2 > newton_tol * newton_tol * scale2)) break;  // converged (or non-finite: stop)
   }
+  return done;
 }
 
 // Correction operator C_mode: 0 none; 1 eq (10);
 // 2 eq (10) then dual scaling; 3 eq (10) then six-integral projection.
 // Order: spins first, then (r, p) with the corrected spins.
-// Returns false only when mode 2 skipped its orbital part.
+// Returns false only when mode 2 skipped its orbital part; *gn_steps (optional)
+// receives the number of Gauss-Newton steps mode 3 took.
 template <class T>
-bool correct(State<T>& z, const Params<T>& P, const Refs<T>& R, int mode, int newton_iters, T newton_tol) {
+bool correct(State<T>& z, const Params<T>& P, const Refs<T>& R, int mode, int newton_iters, T newton_tol,
+             int* gn_steps = nullptr) {
+  if (gn_steps) *gn_steps = 0;
   if (mode >= 1) { z.s1 = unit(z.s1); z.s2 = unit(z.s2); }  // eq (10)
   if (mode == 2) return dual_scaling(z, P, R, newton_iters, newton_tol);
-  if (mode == 3) project_six(z, P, R, newton_iters);
+  if (mode == 3) {
+    const int k = project_six(z, P, R, newton_iters, newton_tol);
+    if (gn_steps) *gn_steps = k;
+  }
   return true;
 }
 
@@ -330,8 +350,8 @@ template <class T> inline bool finite_state(const State<T>& z) {
 struct Options {
   int mode;             // correction mode 0..3
   int renorm_interval;  // steps between shadow renormalisations (BASELINE config 1: 100)
-  int newton_iters;     // fixed Newton iteration count (R6)
-  double newton_tol;    // epsilon of PAPER.md:197, mode 2 convergence flag
+  int newton_iters;     // Newton iteration cap (mode 3) / fixed count (mode 2), R6
+  double newton_tol;    // epsilon of PAPER.md:197: mode 3 termination test, mode 2 convergence flag
   double r_merge, r_escape;  // DESIGN.md R13
 };
 
@@ -341,6 +361,7 @@ template <class T> struct OrbitResult {
   T fli;                 // log10 d(t)/d(0), accumulated over renormalisations
   int32_t status;
   int64_t steps_done;
+  int64_t gn_steps;      // Gauss-Newton steps of mode 3 over all accepted steps, orbit + shadow
 };
 
 template <class T> inline void six_integrals(const State<T>& z, const Params<T>& P, T out[6]) {
@@ -365,21 +386,22 @@ OrbitResult<T> integrate_orbit(State<T> z, const Params<T>& P, T h, int64_t n_st
     Rs = references(zs, P);
   }
   int32_t status = ST_OK, flag = 0;
-  int64_t k = 0;
+  int64_t k = 0, gn_total = 0;
   while (k < n_steps) {
+    int gn = 0, gns = 0;
     State<T> zn = rk4_step(z, h, P);
-    if (!correct(zn, P, R, O.mode, O.newton_iters, T(O.newton_tol))) flag = ST_NEWTON_FLAG;
+    if (!correct(zn, P, R, O.mode, O.newton_iters, T(O.newton_tol), &gn)) flag = ST_NEWTON_FLAG;
     State<T> zsn = zs;
     if (shadow) {
       zsn = rk4_step(zs, h, P);
-      correct(zsn, P, Rs, O.mode, O.newton_iters, T(O.newton_tol));
+      correct(zsn, P, Rs, O.mode, O.newton_iters, T(O.newton_tol), &gns);
     }
     // status check on the completed step (R13); on failure keep the last good state
     if (!finite_state(zn) || !finite_state(zsn)) { status = ST_NONFINITE; break; }
     const T rr = o_sqrt(dot(zn.r, zn.r));
     if (rr < T(O.r_merge)) { status = ST_MERGED; break; }
     if (rr > T(O.r_escape)) { status = ST_UNBOUND; break; }
-    z = zn; zs = zsn; ++k;
+    z = zn; zs = zsn; ++k; gn_total += gn + gns;
     if (shadow && O.renorm_interval > 0 && (k % O.renorm_interval) == 0) {
       const State<T> dz = zs - z;
       const T d = o_sqrt(norm12sq(dz));
@@ -395,6 +417,7 @@ OrbitResult<T> integrate_orbit(State<T> z, const Params<T>& P, T h, int64_t n_st
   out.fli = shadow ? acc + o_log10(o_sqrt(norm12sq(zs - z)) / d0) : T(0);
   out.status = status | flag;
   out.steps_done = k;
+  out.gn_steps = gn_total;
   return out;
 }
 

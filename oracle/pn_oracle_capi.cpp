@@ -103,7 +103,7 @@ void correct_t(int64_t n, const double* states, const ParamArrays& A, const doub
 template <class T>
 void integrate_t(int64_t n, const double* states, const ParamArrays& A, double h, int64_t n_steps,
                  double shadow_eps, const Options& O, double* out_states, double* out_inv, double* out_fli,
-                 int32_t* out_status, int64_t* out_step, int n_threads) {
+                 int32_t* out_status, int64_t* out_step, int64_t* out_gn, int n_threads) {
 #pragma omp parallel for schedule(static) num_threads(n_threads)
   for (int64_t i = 0; i < n; ++i) {
     const State<T> z = load_state<T>(states, n, i);
@@ -118,6 +118,7 @@ void integrate_t(int64_t n, const double* states, const ParamArrays& A, double h
     if (out_fli) out_fli[i] = to_double(R.fli);
     if (out_status) out_status[i] = R.status;
     if (out_step) out_step[i] = R.steps_done;
+    if (out_gn) out_gn[i] = R.gn_steps;
   }
 }
 
@@ -160,22 +161,23 @@ int oracle_integrate(int precision, int64_t n, const double* states, const doubl
                      int64_t n_steps, int mode, double shadow_eps, int renorm_interval, int newton_iters,
                      double newton_tol, double r_merge, double r_escape, double* out_states,
                      double* out_invariants, double* out_fli, int32_t* out_status, int64_t* out_step,
-                     int n_threads) {
+                     int64_t* out_gn_steps, int n_threads) {
   const ParamArrays A = {beta, chi1, chi2, kq1, kq2, terms};
   const Options O = {mode, renorm_interval, newton_iters, newton_tol, r_merge, r_escape};
   if (n_threads <= 0) n_threads = omp_get_max_threads();
   if (precision == 0)
     integrate_t<long double>(n, states, A, h, n_steps, shadow_eps, O, out_states, out_invariants, out_fli,
-                             out_status, out_step, n_threads);
+                             out_status, out_step, out_gn_steps, n_threads);
   else
     integrate_t<double>(n, states, A, h, n_steps, shadow_eps, O, out_states, out_invariants, out_fli,
-                        out_status, out_step, n_threads);
+                        out_status, out_step, out_gn_steps, n_threads);
   return 0;
 }
 
 // Exact flop counts of the oracle's own formulation on one orbit (add, sub, mul,
 // div, sqrt = 1 each): counts[0] = rhs, [1] = rk4_step, [2] = correct(mode),
-// [3] = hamiltonian, [4] = gradient.
+// [3] = hamiltonian, [4] = gradient.  The correction is counted with tolerance 0,
+// i.e. with all newton_iters steps taken.
 int oracle_count_flops(const double* state12, double beta, double chi1, double chi2, double kq1, double kq2,
                        uint32_t terms, int mode, int newton_iters, long long* counts) {
   const State<Counted> z = load_state<Counted>(state12, 1, 0);
@@ -183,7 +185,7 @@ int oracle_count_flops(const double* state12, double beta, double chi1, double c
   const Refs<Counted> R = references(z, P);
   Counted::flops = 0; (void)rhs(z, P); counts[0] = Counted::flops;
   Counted::flops = 0; State<Counted> zn = rk4_step(z, Counted(1.0), P); counts[1] = Counted::flops;
-  Counted::flops = 0; (void)correct(zn, P, R, mode, newton_iters, Counted(1e-10)); counts[2] = Counted::flops;
+  Counted::flops = 0; (void)correct(zn, P, R, mode, newton_iters, Counted(0.0)); counts[2] = Counted::flops;
   Counted::flops = 0; (void)hamiltonian(z, P); counts[3] = Counted::flops;
   Counted::flops = 0; (void)gradient(z, P); counts[4] = Counted::flops;
   return 0;

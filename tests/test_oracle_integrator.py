@@ -211,9 +211,9 @@ def test_mode2_rounding_amplification_sets_the_parity_bound():
 
 
 def test_two_newton_iterations_leave_a_residual_at_deep_periastron():
-    """DESIGN.md section 7 ("deep periastron"): config-2 cell (3, 308) passes periastron at |r| = 2.2 on
-    step 1e4.  With the fixed 2 Newton iterations (R6) the energy residual there is ~7e-11; one step later,
-    and with 4 iterations, it is round-off.  The GPU drift bound is therefore split at |r| = 3."""
+    """DESIGN.md R6 / section 7 ("deep periastron"): config-2 cell (3, 308) passes periastron at |r| = 2.2
+    on step 1e4.  Capped at 2 Newton iterations the energy residual there is ~7e-11; one step later, and
+    with the default cap of 4 (epsilon-terminated), it is round-off."""
     sub = workloads.config2(n_steps=10_000).subset([3 * 314 + 308])
 
     def energy_drift(n, iters):
@@ -226,6 +226,30 @@ def test_two_newton_iterations_leave_a_residual_at_deep_periastron():
     assert 2.0 < r < 2.5 and 1e-12 < d2 < 1e-9
     assert energy_drift(10_001, 2)[0] < 1e-14
     assert energy_drift(10_000, 4)[0] < 1e-14
+    o = oracle.integrate(sub.states, 1.0, 10_000, 3, shadow_eps=1e-8, **sub.params())       # defaults
+    assert abs(oracle.integrals(o.states, **sub.params())[0, 0] / o.invariants[0, 0] - 1) < 1e-14
+
+
+def test_newton_termination_rule_of_mode3():
+    """DESIGN.md R6: Gauss-Newton steps repeat until |(dr,dp)| <= eps |p|, at most
+    newton_iters times.  eps = 0 gives the fixed count (bar exactly-zero steps); eps = 1e-10 stops after the first
+    step on mild orbits and changes the result by O(eps^2) only (quadratic convergence)."""
+    w = workloads.config0(16)
+    n_steps = 400
+    fixed = oracle.integrate(w.states, 1.0, n_steps, 3, newton_iters=3, newton_tol=0.0, **w.params())
+    # eps = 0: only an exactly vanishing step (possible on the third iteration) ends the loop early
+    assert (fixed.gn_steps > 2.9 * n_steps).all() and (fixed.gn_steps <= 3 * n_steps).all()
+    eps = oracle.integrate(w.states, 1.0, n_steps, 3, newton_iters=3, newton_tol=1e-10, **w.params())
+    assert (eps.gn_steps >= n_steps).all() and (eps.gn_steps <= 2 * n_steps).all()
+    assert (eps.gn_steps < 3 * n_steps).all()
+    assert _per_orbit_rel_err(eps.states, fixed.states).max() < 1e-15
+    loose = oracle.integrate(w.states, 1.0, n_steps, 3, newton_iters=3, newton_tol=1.0, **w.params())
+    assert (loose.gn_steps == n_steps).all()                            # the first step is always taken
+    sh = oracle.integrate(w.states[:, :4], 1.0, 100, 3, shadow_eps=1e-8, newton_iters=2, newton_tol=0.0,
+                          **w.subset(np.arange(4)).params())
+    assert (sh.gn_steps == 2 * 2 * 100).all()                           # orbit + shadow, both steps non-zero
+    for mode in (0, 1, 2):
+        assert (oracle.integrate(w.states[:, :2], 1.0, 10, mode, **w.subset(np.arange(2)).params()).gn_steps == 0).all()
 
 
 def test_flop_counter_reports_the_oracles_own_formulation():

@@ -3,6 +3,7 @@
 
 One "step" = one pass of the whole hot path (mc_integrate: load, 1e5 x [RK4 + six-integral correction]
 on orbit and shadow, FLI renormalisation every 100 steps, status, store) over the 314 x 314 grid.
+`value` counts accepted orbit-steps (dropped cells stop counting when they freeze).
 N > 1 (torchrun): the global grid has 314*N rows of r0, sharded by contiguous row ranges, no
 collective on the data path (weak scaling).  `--impl reference` times the CPU oracle instead.
 Prints ONE JSON line on rank 0.  See DESIGN.md section 8 for every number's definition.
@@ -24,11 +25,15 @@ from paper_1802_00147_b200 import sharding, workloads  # noqa: E402
 
 METRIC = "orbit-RK4-steps/sec (with correction+FLI)"
 UNIT = "orbit-steps/s"
-# Algorithmic FP64 flops of one orbit-step (orbit + shadow, mode 3 with 2 Newton iterations, QM off),
-# FMA = 2, add/mul/rsqrt/rcp = 1: 2 x [4 x 229 (RHS) + 168 (RK4 sums) + 800 (correction) + 5 (|r|^2)].
-# Hand count of the kernel's own formulation, itemised in DESIGN.md section 6; the oracle's unfactored
-# formulation needs 8018 (oracle.count_flops), so this is the conservative figure.
-FLOP_PER_ORBIT_STEP = 3778.0
+# Algorithmic FP64 flops (FMA = 2, add/mul/rsqrt/rcp = 1; QM off), itemised in DESIGN.md section 8:
+#   per orbit-step (orbit + shadow), without the Gauss-Newton steps of mode 3:
+#     2 x [4 x 229 (RHS) + 168 (RK4 sums) + 34 (eq 10) + 12 (L_t) + 5 (|r|^2 status test)] = 2270
+#   per Gauss-Newton step (gradient + H 190, residuals/Schur/solve/update 187, termination test 13) = 390
+# The number of Gauss-Newton steps is data dependent (epsilon-terminated, R6): the kernel counts
+# them (mc_get_work) and the flop total of a launch is 2270 x accepted orbit-steps + 390 x counted steps.
+# The oracle's unfactored formulation needs about twice as much (oracle.count_flops): conservative.
+FLOP_PER_ORBIT_STEP_BASE = 2270.0
+FLOP_PER_GN_STEP = 390.0
 FP64_LANES_PER_SM = 64
 
 
@@ -216,7 +221,6 @@ def run_mc(args):
     kernel_ms = [a.elapsed_time(b) for a, b in ev]
     dev_ms = float(sum(kernel_ms))
     dev_ms_max = sharding.max_over_ranks(dev_ms, dev)
-    value = orbit_steps_rank * world * args.steps / (dev_ms_max * 1e-3)
 
     # end to end through the C ABI with HOST buffers (pinned): H2D + kernel + D2H inside the timed call
     z_host = z_pin.numpy()
@@ -227,13 +231,19 @@ def run_mc(args):
         hres = I.integrate_host(z_host, w.h, w.n_steps, w.correction_mode, shadow_eps=w.shadow_eps)
     barrier()
     e2e_s = time.perf_counter() - t0
-    e2e_value = orbit_steps_rank * world * args.steps / sharding.max_over_ranks(e2e_s, dev)
+    e2e_s_max = sharding.max_over_ranks(e2e_s, dev)
     h2d = 12 * 8 * n
     d2h = (12 + 12 + 1) * 8 * n + 4 * n + 8 * n
 
     info = I.launch_info()
     status = res.status.cpu().numpy()
     fli = res.fli.cpu().numpy()
+    steps_done = float(res.steps_done.sum().item())          # accepted orbit-steps of one launch (this rank)
+    gn_steps = float(I.work(n).sum().item())                  # Gauss-Newton steps of one launch, orbit + shadow
+    steps_done_job = sharding.sum_over_ranks(steps_done, dev)
+    # orbit-steps actually integrated (dropped cells stop counting when they freeze), whole job
+    value = steps_done_job * args.steps / (dev_ms_max * 1e-3)
+    e2e_value = steps_done_job * args.steps / e2e_s_max
     I.close()
     if rank != 0:
         if world > 1:
@@ -244,14 +254,17 @@ def run_mc(args):
     sm_max = float(mp.get("sm_max_mhz", clocks.get("sm_max_mhz") or 1965.0))
     nominal_tf = info["num_sms"] * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     per_launch_s = (dev_ms / args.steps) * 1e-3
-    achieved_tf = FLOP_PER_ORBIT_STEP * orbit_steps_rank / per_launch_s / 1e12
+    flop_per_launch = FLOP_PER_ORBIT_STEP_BASE * steps_done + FLOP_PER_GN_STEP * gn_steps
+    achieved_tf = flop_per_launch / per_launch_s / 1e12
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": nominal_tf, "unit": "TFLOP/s",
                 "frac": achieved_tf / nominal_tf, "traffic": None,
                 "peak_source": f"derived: {info['num_sms']} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x {sm_max:.0f} MHz "
                                "(MEASURED_PEAKS.json has no FP64 entry)",
                 "peak_measured_dfma": peak_tf, "frac_of_measured_dfma": achieved_tf / peak_tf if peak_tf else None,
                 "dfma_probe_implied_sm_mhz": peak_clock,
-                "flop_per_orbit_step": FLOP_PER_ORBIT_STEP, "kernel": "mc::integrate_kernel<uniform,QM off,mode 3>",
+                "flop_per_launch": flop_per_launch, "flop_per_orbit_step": flop_per_launch / max(steps_done, 1.0),
+                "gn_steps_per_trajectory_step": gn_steps / max(2.0 * steps_done, 1.0),
+                "accepted_orbit_steps_per_launch": steps_done, "kernel": "mc::integrate_kernel<uniform,QM off,mode 3>",
                 "kernel_ms_per_launch": dev_ms / args.steps,
                 "regs_per_thread": info["regs_per_thread"], "spill_bytes": info["local_bytes"],
                 "blocks_per_sm": info["blocks_per_sm"], "grid": info["grid"], "block": info["block"]}
@@ -260,8 +273,9 @@ def run_mc(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"config2: {args.grid}x{args.grid} orbit scan per GPU (r0 in [10,60] x theta in [0,pi]), "
                                    f"equal mass, chi=1, N+1PN+2PN+SO+SS, RK4 h=1, {w.n_steps} steps, shadow 1e-8 "
-                                   "renormalised every 100 steps + FLI, six-integral correction (mode 3, 2 Newton iterations)",
-                       "orbits_per_gpu": n, "rk4_steps": w.n_steps, "l2": "flushed (256 MiB write) between timed iterations",
+                                   "renormalised every 100 steps + FLI, six-integral correction (mode 3, Gauss-Newton terminated at eps=1e-10, cap 4)",
+                       "orbits_per_gpu": n, "rk4_steps": w.n_steps,
+                       "orbit_steps_counted": "accepted steps (sum of steps_done); scheduled = orbits x rk4_steps = %d" % int(orbit_steps_rank * world), "l2": "flushed (256 MiB write) between timed iterations",
                        "parallelism": f"orbit-sharded x{world}, no collective"},
             "clocks": clocks, "wall_s_timed_region": t_wall,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},

@@ -71,15 +71,18 @@ typedef struct mc_params {
   const double* d_kq1;
   const double* d_kq2;
   int32_t renorm_interval; /* steps between shadow renormalisations, > 0 (BASELINE config 1: 100)          */
-  int32_t newton_iters;    /* fixed Newton iteration count, 1..16 (R6); default 2                */
-  double newton_tol;       /* epsilon of PAPER.md:197 (1e-10): mode 2 convergence test on |dv|             */
+  int32_t newton_iters;    /* Newton iterations, 1..16 (R6): the cap of mode 3, the fixed count of
+                              mode 2; default 4                                                             */
+  double newton_tol;       /* epsilon of PAPER.md:197 (default 1e-10).  Mode 3: a Gauss-Newton step with
+                              |(dr,dp)|_2 <= epsilon |p|_2 is the last one; 0 = always newton_iters steps.
+                              Mode 2: the scaling is skipped unless the last |dv| <= epsilon               */
   double r_merge;          /* default 2    (R13)                                                 */
   double r_escape;         /* default 1e4                                                                  */
   void* cuda_stream;       /* cudaStream_t all work is enqueued on (e.g. torch's current stream); NULL = 0 */
 } mc_params;
 
 /* Fill *p with defaults: terms = 1PN|2PN|SO|S1S2, device 0, uniform beta = chi = kq = 1,
- * renorm_interval 100, newton_iters 2, newton_tol 1e-10, r_merge 2, r_escape 1e4, stream NULL. */
+ * renorm_interval 100, newton_iters 4, newton_tol 1e-10, r_merge 2, r_escape 1e4, stream NULL. */
 int mc_params_default(mc_params* p);
 
 /* Validate params, select the device, allocate the handle.  *out_handle is set only on success. */
@@ -120,6 +123,11 @@ int mc_integrate_host(mc_handle* h, const double* states, int64_t n_orbits, doub
  * DEVICE arrays of the caller: out_status int32[n_orbits] (mc_status), out_step int64[n_orbits] =
  * number of completed steps.  Either pointer may be NULL. */
 int mc_get_status(mc_handle* h, int32_t* out_status, int64_t* out_step);
+
+/* Work done by the most recent mc_integrate on this handle: out_gn_steps, DEVICE int64[n_orbits] = number
+ * of Gauss-Newton steps correction mode 3 took over all accepted steps of the orbit and its shadow
+ * (0 for the other modes).  Stream-ordered copy.  bench.py derives the algorithmic flop count from it. */
+int mc_get_work(mc_handle* h, int64_t* out_gn_steps);
 
 /* Evaluate pieces of the model on the device with the handle's parameters (used by the parity tests
  * to compare the kernel's fused routines with the oracle one by one).  states: DEVICE double[12][n].

@@ -16,7 +16,7 @@ TERMS_DEFAULT = MC_TERM_1PN | MC_TERM_2PN | MC_TERM_SO | MC_TERM_S1S2
 MC_OK, MC_EINVAL, MC_ECUDA, MC_EARCH, MC_ENOMEM = 0, -1, -2, -3, -4
 
 # every symbol include/mc.h declares (tests/test_abi.py checks the header against this list)
-EXPORTS = ["mc_params_default", "mc_create", "mc_integrate", "mc_integrate_host", "mc_get_status", "mc_eval",
+EXPORTS = ["mc_params_default", "mc_create", "mc_integrate", "mc_integrate_host", "mc_get_status", "mc_get_work", "mc_eval",
            "mc_last_launch_info", "mc_fp64_peak", "mc_destroy", "mc_strerror"]
 
 
@@ -76,6 +76,7 @@ def load_library():
     lib.mc_integrate.argtypes = [vp, vp, i64, dbl, i64, i32, dbl, vp, vp, vp]
     lib.mc_integrate_host.argtypes = [vp, vp, i64, dbl, i64, i32, dbl, vp, vp, vp, vp, vp]
     lib.mc_get_status.argtypes = [vp, vp, vp]
+    lib.mc_get_work.argtypes = [vp, vp]
     lib.mc_eval.argtypes = [vp, i32, vp, i64, dbl, i32, vp, vp]
     lib.mc_last_launch_info.argtypes = [vp, ctypes.POINTER(mc_launch_info)]
     lib.mc_fp64_peak.argtypes = [i32, dbl, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
@@ -120,7 +121,7 @@ class Integrator:
     """mc_create / mc_integrate / mc_destroy with torch tensors as device buffers."""
 
     def __init__(self, terms=TERMS_DEFAULT, beta=1.0, chi1=1.0, chi2=1.0, kq1=1.0, kq2=1.0, device=0,
-                 renorm_interval=100, newton_iters=2, newton_tol=1e-10, r_merge=2.0, r_escape=1e4, stream=None):
+                 renorm_interval=100, newton_iters=4, newton_tol=1e-10, r_merge=2.0, r_escape=1e4, stream=None):
         import torch
         self._torch = torch
         self._lib = load_library()
@@ -218,6 +219,13 @@ class Integrator:
         r = self._dev(refs) if refs is not None else None
         _check(self._lib.mc_eval(self._h, code, z.data_ptr(), n, float(h), int(mode),
                                  r.data_ptr() if r is not None else None, out.data_ptr()))
+        return out
+
+    def work(self, n):
+        """mc_get_work: Gauss-Newton steps per orbit (orbit + shadow) of the last integrate -> int64 tensor (n,)."""
+        torch = self._torch
+        out = torch.empty(n, dtype=torch.int64, device=self.device)
+        _check(self._lib.mc_get_work(self._h, out.data_ptr()))
         return out
 
     def launch_info(self) -> dict:

@@ -54,7 +54,7 @@ struct mc_handle {
   cudaStream_t stream;
   int num_sms;
   int64_t last_n;            // orbits of the last mc_integrate (status buffers valid for these)
-  DeviceBuf status, step;    // int32[n], int64[n]
+  DeviceBuf status, step, gn;   // int32[n], int64[n], int64[n]
   DeviceBuf h_in, h_out, h_inv, h_fli;   // scratch of mc_integrate_host
   mc_launch_info info;
 };
@@ -104,9 +104,10 @@ eval_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ mc::Int
     mc::Refs R;
     R.E0 = refs[o];
     R.J0[0] = refs[A.n + o]; R.J0[1] = refs[2 * A.n + o]; R.J0[2] = refs[3 * A.n + o];
-    if (mode == 1) mc::correct<1, QM>(c, z, R, A.newton_iters, A.newton_tol);
-    else if (mode == 2) mc::correct<2, QM>(c, z, R, A.newton_iters, A.newton_tol);
-    else if (mode == 3) mc::correct<3, QM>(c, z, R, A.newton_iters, A.newton_tol);
+    int gn;
+    if (mode == 1) mc::correct<1, QM>(c, z, R, A.newton_iters, A.newton_tol, gn);
+    else if (mode == 2) mc::correct<2, QM>(c, z, R, A.newton_iters, A.newton_tol, gn);
+    else if (mode == 3) mc::correct<3, QM>(c, z, R, A.newton_iters, A.newton_tol, gn);
 #pragma unroll
     for (int i = 0; i < 12; ++i) f[i] = z[i];
   }
@@ -162,7 +163,7 @@ int mc_params_default(mc_params* p) {
   p->per_orbit = 0;
   p->beta = p->chi1 = p->chi2 = p->kq1 = p->kq2 = 1.0;
   p->renorm_interval = 100;
-  p->newton_iters = 2;
+  p->newton_iters = 4;
   p->newton_tol = 1e-10;
   p->r_merge = 2.0;
   p->r_escape = 1e4;
@@ -217,11 +218,13 @@ int mc_integrate(mc_handle* h, const double* states, int64_t n_orbits, double st
   if (rc) return rc;
   rc = h->step.reserve(sizeof(int64_t) * (size_t)n_orbits);
   if (rc) return rc;
+  rc = h->gn.reserve(sizeof(int64_t) * (size_t)n_orbits);
+  if (rc) return rc;
 
   mc::IntegrateArgs A;
   fill_args(h, A);
   A.states = states; A.out_states = out_states; A.out_inv = out_invariants; A.out_fli = shadow ? out_fli : nullptr;
-  A.out_status = (int32_t*)h->status.p; A.out_step = (int64_t*)h->step.p;
+  A.out_status = (int32_t*)h->status.p; A.out_step = (int64_t*)h->step.p; A.out_gn = (int64_t*)h->gn.p;
   A.n = n_orbits; A.n_steps = n_steps; A.h = step_h; A.shadow_eps = shadow_eps;
 
   const bool qm = (h->P.terms & MC_TERM_QM) != 0;
@@ -257,6 +260,14 @@ int mc_get_status(mc_handle* h, int32_t* out_status, int64_t* out_step) {
     MC_CUDA(cudaMemcpyAsync(out_status, h->status.p, sizeof(int32_t) * (size_t)h->last_n, cudaMemcpyDeviceToDevice, h->stream));
   if (out_step)
     MC_CUDA(cudaMemcpyAsync(out_step, h->step.p, sizeof(int64_t) * (size_t)h->last_n, cudaMemcpyDeviceToDevice, h->stream));
+  return MC_OK;
+}
+
+int mc_get_work(mc_handle* h, int64_t* out_gn_steps) {
+  if (!h || !out_gn_steps) return MC_EINVAL;
+  if (h->last_n == 0) return MC_OK;
+  MC_CUDA(cudaSetDevice(h->P.device));
+  MC_CUDA(cudaMemcpyAsync(out_gn_steps, h->gn.p, sizeof(int64_t) * (size_t)h->last_n, cudaMemcpyDeviceToDevice, h->stream));
   return MC_OK;
 }
 
@@ -354,7 +365,7 @@ int mc_fp64_peak(int32_t device, double millis, double* out_tflops, double* out_
 int mc_destroy(mc_handle* h) {
   if (!h) return MC_EINVAL;
   cudaSetDevice(h->P.device);
-  h->status.release(); h->step.release();
+  h->status.release(); h->step.release(); h->gn.release();
   h->h_in.release(); h->h_out.release(); h->h_inv.release(); h->h_fli.release();
   delete h;
   return MC_OK;

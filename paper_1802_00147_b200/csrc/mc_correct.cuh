@@ -20,61 +20,75 @@ __device__ __forceinline__ void references(const C& c, const double* z, Refs& R)
 // M^-1 is closed-form (Woodbury): M^-1 x = N(x)/D, D = (r.r + p.p) |L|^2,
 //   N(x) = |L|^2 x + r (rr (r.x) + rp (p.x)) + p (rp (r.x) + pp (p.x)),
 // so the 4x4 solve needs one reciprocal.  The oracle solves the same system by pivoted elimination.
+// Iteration control (R6): a lane repeats the step until its last update
+// satisfies |(dr,dp)|^2 <= tol^2 p.p, at most `iters` times.  The decision is per lane (results do not
+// depend on the neighbours); the warp leaves the loop when no lane needs another step.  Must be called
+// by all 32 lanes.  Returns the number of steps this lane took.
 template <bool QM, class C>
-__device__ __forceinline__ void project_six(const C& c, double* z, const Refs& R, int iters) {
+__device__ __forceinline__ int project_six(const C& c, double* z, const Refs& R, int iters, double tol2) {
   double Lt[3];
 #pragma unroll
   for (int i = 0; i < 3; ++i) Lt[i] = fma(-c[K_S2], z[9 + i], fma(-c[K_S1], z[6 + i], R.J0[i]));
+  bool need = true;
+  int done = 0;
 #pragma unroll 1
   for (int it = 0; it < iters; ++it) {
-    double g[12], H;
-    pn_eval<QM, false, true>(c, z, g, H);
-    double* r = z;
-    double* p = z + 3;
-    const double* a = g;
-    const double* b = g + 3;
-    double fL[3], cv[3], t[3];
-    cross3(r, p, fL);
+    if (!__any_sync(0xffffffffu, need)) break;
+    if (need) {
+      double g[12], H;
+      pn_eval<QM, false, true>(c, z, g, H);
+      double* r = z;
+      double* p = z + 3;
+      const double* a = g;
+      const double* b = g + 3;
+      double fL[3], cv[3];
+      cross3(r, p, fL);
 #pragma unroll
-    for (int i = 0; i < 3; ++i) fL[i] -= Lt[i];
-    const double f0 = H - R.E0;
-    cross3(a, p, cv);
-    cross3(r, b, t);
+      for (int i = 0; i < 3; ++i) fL[i] -= Lt[i];
+      const double f0 = H - R.E0;
+      // c = a x p + r x b
+      cv[0] = fma(r[1], b[2], fma(-r[2], b[1], fma(a[1], p[2], -(a[2] * p[1]))));
+      cv[1] = fma(r[2], b[0], fma(-r[0], b[2], fma(a[2], p[0], -(a[0] * p[2]))));
+      cv[2] = fma(r[0], b[1], fma(-r[1], b[0], fma(a[0], p[1], -(a[1] * p[0]))));
+      const double gg = dot3(a, a) + dot3(b, b);
+      const double rr = dot3(r, r), pp = dot3(p, p), rp = dot3(r, p);
+      const double LL = fma(rr, pp, -(rp * rp));
+      const double D = (rr + pp) * LL;
+      // N(c), N(fL)
+      const double rc = dot3(r, cv), pc = dot3(p, cv), rf = dot3(r, fL), pf = dot3(p, fL);
+      const double cr_ = fma(rp, pc, rr * rc), cp_ = fma(pp, pc, rp * rc);
+      const double fr_ = fma(rp, pf, rr * rf), fp_ = fma(pp, pf, rp * rf);
+      double Nc[3], Nf[3];
 #pragma unroll
-    for (int i = 0; i < 3; ++i) cv[i] += t[i];
-    const double gg = dot3(a, a) + dot3(b, b);
-    const double rr = dot3(r, r), pp = dot3(p, p), rp = dot3(r, p);
-    const double LL = fma(rr, pp, -(rp * rp));
-    const double D = (rr + pp) * LL;
-    // N(c), N(fL)
-    const double rc = dot3(r, cv), pc = dot3(p, cv), rf = dot3(r, fL), pf = dot3(p, fL);
-    const double cr_ = fma(rp, pc, rr * rc), cp_ = fma(pp, pc, rp * rc);
-    const double fr_ = fma(rp, pf, rr * rf), fp_ = fma(pp, pf, rp * rf);
-    double Nc[3], Nf[3];
+      for (int i = 0; i < 3; ++i) {
+        Nc[i] = fma(p[i], cp_, fma(r[i], cr_, LL * cv[i]));
+        Nf[i] = fma(p[i], fp_, fma(r[i], fr_, LL * fL[i]));
+      }
+      const double S = fma(gg, D, -dot3(cv, Nc));
+      const double num = fma(D, f0, -dot3(cv, Nf));
+      const double DS = D * S;
+      const double inv = (DS != 0.0) ? rcp_nz(DS) : 0.0;      // singular only for r || p or a circular orbit
+      const double l0 = num * D * inv;                         // num / S
+      const double sD = S * inv;                               // 1 / D
+      double lL[3], d1[3], d2[3];
 #pragma unroll
-    for (int i = 0; i < 3; ++i) {
-      Nc[i] = fma(p[i], cp_, fma(r[i], cr_, LL * cv[i]));
-      Nf[i] = fma(p[i], fp_, fma(r[i], fr_, LL * fL[i]));
-    }
-    const double S = fma(gg, D, -dot3(cv, Nc));
-    const double num = fma(D, f0, -dot3(cv, Nf));
-    const double DS = D * S;
-    const double inv = (DS != 0.0) ? rcp_nz(DS) : 0.0;      // singular only for r || p or a circular orbit
-    const double l0 = num * D * inv;                         // num / S
-    const double sD = S * inv;                               // 1 / D
-    double lL[3], d1[3], d2[3];
+      for (int i = 0; i < 3; ++i) lL[i] = fma(-l0, Nc[i], Nf[i]) * sD;
+      cross3(p, lL, d1);   // dr = l0 a + p x lL
+      cross3(lL, r, d2);   // dp = l0 b + lL x r
+      double dd = 0.0;
 #pragma unroll
-    for (int i = 0; i < 3; ++i) lL[i] = fma(-l0, Nc[i], Nf[i]) * sD;
-    cross3(p, lL, d1);   // dr = l0 a + p x lL
-    cross3(lL, r, d2);   // dp = l0 b + lL x r
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-      const double dr = fma(l0, a[i], d1[i]);
-      const double dp = fma(l0, b[i], d2[i]);
-      r[i] -= dr;
-      p[i] -= dp;
+      for (int i = 0; i < 3; ++i) {
+        const double dr = fma(l0, a[i], d1[i]);
+        const double dp = fma(l0, b[i], d2[i]);
+        dd = fma(dr, dr, fma(dp, dp, dd));
+        r[i] -= dr;
+        p[i] -= dp;
+      }
+      ++done;
+      need = dd > tol2 * pp;       // false also for a non-finite step
     }
   }
+  return done;
 }
 
 // Mode 2: the paper's dual scaling p <- alpha p*, r <- beta_s r* (eq 11) solving H = E0, |J| = |J0|
@@ -136,11 +150,13 @@ __device__ __forceinline__ bool dual_scaling(const C& c, double* z, const Refs& 
 }
 
 // C_mode: spins first (eq 10), then (r,p) with the corrected spins.
+// gn_steps receives the number of Gauss-Newton steps mode 3 took (0 otherwise).
 template <int MODE, bool QM, class C>
-__device__ __forceinline__ bool correct(const C& c, double* z, const Refs& R, int iters, double tol) {
+__device__ __forceinline__ bool correct(const C& c, double* z, const Refs& R, int iters, double tol, int& gn_steps) {
+  gn_steps = 0;
   if (MODE >= 1) { normalise3(z + 6); normalise3(z + 9); }
   if (MODE == 2) return dual_scaling<QM>(c, z, R, iters, tol);
-  if (MODE == 3) project_six<QM>(c, z, R, iters);
+  if (MODE == 3) gn_steps = project_six<QM>(c, z, R, iters, tol * tol);
   return true;
 }
 

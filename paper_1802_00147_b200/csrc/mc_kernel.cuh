@@ -17,6 +17,7 @@ struct IntegrateArgs {
   double* out_fli;           // [n] or null
   int32_t* out_status;       // [n]
   int64_t* out_step;         // [n]
+  int64_t* out_gn;           // [n] Gauss-Newton steps of mode 3 over accepted steps, orbit + shadow
   const double* beta; const double* chi1; const double* chi2; const double* kq1; const double* kq2;  // per-orbit mode
   int64_t n;                 // orbits
   int64_t n_steps;
@@ -92,6 +93,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
   int status = ST_OK, flag = 0;
   bool frozen = false;
   int64_t steps = 0;
+  unsigned long long gn_total = 0;
   double acc = 0.0;
   int until_renorm = A.renorm_interval;
 
@@ -99,7 +101,8 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
   for (int64_t k = 0; k < A.n_steps; ++k) {
     double z[12];
     rk4_step<QM>(c, y, A.h, z);
-    const bool ok = correct<MODE, QM>(c, z, R, A.newton_iters, A.newton_tol);
+    int gn;
+    const bool ok = correct<MODE, QM>(c, z, R, A.newton_iters, A.newton_tol, gn);
     if (MODE == 2 && !ok && !role_shadow && !frozen) flag = ST_NEWTON_FLAG;
     // status of the completed step (R13): non-finite anywhere in the pair, else |r| of the main
     int code = ST_OK;
@@ -117,6 +120,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
 #pragma unroll
         for (int i = 0; i < 12; ++i) y[i] = z[i];
         ++steps;
+        gn_total += (unsigned)gn;
       } else {
         frozen = true;
         status = code;
@@ -152,6 +156,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
   }
 
   // epilogue: FLI from the final separation, invariants, coalesced SoA stores
+  if (shadow) gn_total += __shfl_xor_sync(0xffffffffu, gn_total, 1);
   if (shadow) {
     double ym[12];
 #pragma unroll
@@ -174,6 +179,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
     }
     A.out_status[orbit] = status | flag;
     A.out_step[orbit] = steps;
+    A.out_gn[orbit] = (int64_t)gn_total;
   }
 }
 

@@ -31,6 +31,17 @@ def max_over_ranks(value: float, device=None) -> float:
     return float(t.item())
 
 
+def sum_over_ranks(value: float, device=None) -> float:
+    """all_reduce(SUM) of one float64 scalar; identity when torch.distributed is not initialised."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(value)
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
 def job_throughput(units_per_rank: float, world_size: int, n_timed: int, local_ms: float, device=None) -> float:
     """Whole-job units/s: all ranks' units over the slowest rank's device time (bench.py contract)."""
     return units_per_rank * world_size * n_timed / (max_over_ranks(local_ms, device) * 1e-3)

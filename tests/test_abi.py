@@ -38,7 +38,7 @@ def test_header_is_plain_c(tmp_path):
 def test_params_default_and_struct_size_agree():
     p = binding.params_default()
     assert p.struct_size == ctypes.sizeof(binding.mc_params)
-    assert p.terms == 15 and p.renorm_interval == 100 and p.newton_iters == 2
+    assert p.terms == 15 and p.renorm_interval == 100 and p.newton_iters == 4
     assert p.newton_tol == 1e-10 and p.r_merge == 2.0 and p.r_escape == 1e4
     assert p.beta == p.chi1 == p.chi2 == p.kq1 == p.kq2 == 1.0
 

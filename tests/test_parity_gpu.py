@@ -134,6 +134,7 @@ def test_config1_shadow_fli_parity_per_orbit_params(mc, mode):
     w = workloads.config1().subset(np.arange(150))
     with mc.Integrator(terms=w.terms, **{k: v for k, v in w.params().items() if k != "terms"}) as I:
         g = I.integrate(w.states, w.h, 2000, mode, shadow_eps=w.shadow_eps)
+        work = I.work(w.n_orbits).cpu().numpy()
     o = oracle.integrate(w.states, w.h, 2000, mode, shadow_eps=w.shadow_eps, **w.params())
     assert rel_state_err(g.states.cpu().numpy(), o.states) <= 4 * STATE_RTOL   # 2e3 steps
     assert np.abs(g.fli.cpu().numpy() - o.fli).max() < 1e-3
@@ -141,6 +142,12 @@ def test_config1_shadow_fli_parity_per_orbit_params(mc, mode):
     assert np.array_equal(g.steps_done.cpu().numpy(), o.steps_done)
     if mode == 3:
         assert drift(g.states.cpu().numpy(), o.invariants[0:6], **w.params()) <= DRIFT_TOL
+        # Gauss-Newton step counts (epsilon-terminated, R6): the termination test is taken in FP64 here and in
+        # long double in the oracle, so single decisions at the threshold may differ
+        assert np.abs(work - o.gn_steps).max() <= 0.01 * o.gn_steps.max()
+        assert (work >= 2 * 2000).all() and (work < 2 * 2 * 2000).all()
+    else:
+        assert (work == 0).all()
 
 
 def classes(fli, status):
@@ -286,16 +293,11 @@ def test_full_size_scan_sampled_against_oracle(mc):
     live = gs == 0
     assert 0.85 < live.mean() < 1.0
     inv0 = g.invariants.cpu().numpy()[0:6]
-    # Cells that end the run at a deep periastron (final |r| < 3, just above r_merge = 2) have just taken an
-    # RK4 step whose error is too large for two Newton iterations to remove completely: the oracle itself
-    # shows 7e-11 on cell (3, 308) at step 1e4 and 2e-16 one step later ("deep
-    # periastron"; tests/test_oracle_integrator.py::test_two_newton_iterations_leave_a_residual_at_deep_periastron).
-    rfin = np.linalg.norm(gz[0:3], axis=0)
-    calm, plunging = live & (rfin >= 3.0), live & (rfin < 3.0)
-    assert plunging.sum() < 0.005 * live.sum()
-    assert drift(gz[:, calm], inv0[:, calm], **w.subset(np.where(calm)[0]).params()) <= DRIFT_TOL
-    if plunging.any():
-        assert drift(gz[:, plunging], inv0[:, plunging], **w.subset(np.where(plunging)[0]).params()) <= 1e-7
+    # Every live cell, including those that end the run at a deep periastron (|r| < 3): with the Newton cap
+    # of 4 (R6) the residual that 2 iterations leave there (7e-11, pinned in tests/test_oracle_integrator.py::
+    # test_two_newton_iterations_leave_a_residual_at_deep_periastron) is removed.
+    assert (np.linalg.norm(gz[0:3], axis=0)[live] < 3.0).sum() > 20           # the case has such cells
+    assert drift(gz[:, live], inv0[:, live], **w.subset(np.where(live)[0]).params()) <= DRIFT_TOL
     rng = np.random.default_rng(2)
     idx = np.sort(np.concatenate([rng.choice(314 * 314, 40, replace=False), rng.choice(314 * 40, 8, replace=False)]))
     sub = w.subset(idx)

@@ -107,7 +107,7 @@ int mc_create(const mc_params* params, mc_handle** out_handle);
  * host<->device copy.  All buffers are owned by the caller.  n_orbits = 0 or n_steps = 0 are valid
  * (n_steps = 0 copies the normalised state and evaluates the invariants).  Numerical failures of
  * single orbits are not errors: see mc_get_status.
- * Errors: MC_EINVAL (null/negative arguments, unknown mode, non-finite step_h), MC_ECUDA. */
+ * Errors: MC_EINVAL (null/negative arguments, n_steps >= 2^31, unknown mode, non-finite step_h), MC_ECUDA. */
 int mc_integrate(mc_handle* h, const double* states, int64_t n_orbits, double step_h, int64_t n_steps,
                  int32_t correction_mode, double shadow_eps, double* out_states,
                  double* out_invariants, double* out_fli);

@@ -205,7 +205,7 @@ int mc_create(const mc_params* params, mc_handle** out_handle) {
 int mc_integrate(mc_handle* h, const double* states, int64_t n_orbits, double step_h, int64_t n_steps,
                  int32_t correction_mode, double shadow_eps, double* out_states, double* out_invariants,
                  double* out_fli) {
-  if (!h || n_orbits < 0 || n_steps < 0) return MC_EINVAL;
+  if (!h || n_orbits < 0 || n_steps < 0 || n_steps > 0x7fffffffLL) return MC_EINVAL;
   if (correction_mode < 0 || correction_mode > 3) return MC_EINVAL;
   if (!std::isfinite(step_h) || !std::isfinite(shadow_eps)) return MC_EINVAL;
   const bool shadow = shadow_eps != 0.0;

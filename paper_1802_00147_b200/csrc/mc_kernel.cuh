@@ -92,13 +92,14 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
 
   int status = ST_OK, flag = 0;
   bool frozen = false;
-  int64_t steps = 0;
+  int steps = 0;            // n_steps < 2^31 (mc_integrate checks)
   unsigned long long gn_total = 0;
   double acc = 0.0;
   int until_renorm = A.renorm_interval;
 
+  const int n_steps = (int)A.n_steps;
 #pragma unroll 1
-  for (int64_t k = 0; k < A.n_steps; ++k) {
+  for (int k = 0; k < n_steps; ++k) {
     double z[12];
     rk4_step<QM>(c, y, A.h, z);
     int gn;

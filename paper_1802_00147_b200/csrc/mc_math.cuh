@@ -77,24 +77,24 @@ __device__ __forceinline__ void pn_eval(const C& c, const double* z, double* g, 
   const double u2 = u * u, u3 = u2 * u, u5 = u3 * u2;
   const double rp = dot3(r, p);
   const double P = dot3(p, p);
-  const double npu = rp * u;
-  const double Q = npu * npu;
+  const double w = rp * u2;                                        // (n.p) u
+  const double Q = rp * w;                                         // (n.p)^2
 
-  // orbital polynomials (Horner)
+  // orbital polynomials (Horner); every constant multiple is precomputed (mc_consts.h)
   const double t1 = fma(c[K_D2], Q, fma(c[K_D1], P, c[K_B1]));   // b1 + d1 P + d2 Q
   const double t2 = fma(c[K_D3], Q, c[K_B2]);                    // b2 + d3 Q
   const double t3 = fma(c[K_E2], Q, c[K_E1] * P);                // e1 P + e2 Q
   // H_P = 1/2 + P (2 a1 + 3 c3 P) + u (b1 + 2 d1 P + d2 Q + e1 u)
   const double hp_u = fma(c[K_E1], u, fma(c[K_D1], P, t1));
-  const double HP = fma(u, hp_u, fma(P, fma(3.0 * c[K_C3], P, 2.0 * c[K_A1]), 0.5));
-  // H_Q = u (b2 + d2 P + 2 d3 Q + e2 u)
-  const double HQ = u * fma(c[K_E2], u, fma(c[K_D2], P, fma(c[K_D3], Q, t2)));
+  const double HP = fma(u, hp_u, fma(P, fma(c[K_3C3], P, c[K_2A1]), 0.5));
+  // 2 H_Q = u (2 b2 + 2 d2 P + 4 d3 Q + 2 e2 u)
+  const double HQ2 = u * fma(c[K_4D3], Q, fma(c[K_2D2], P, fma(c[K_2E2], u, c[K_2B2])));
   // H_u = -1 + P t1 + Q t2 + u (2 h1 + 2 t3 + 3 f1 u)
-  const double hu_u = fma(3.0 * c[K_F1], u, fma(2.0, t3, 2.0 * c[K_H1]));
+  const double hu_u = fma(c[K_3F1], u, fma(2.0, t3, c[K_2H1]));
   const double Hu = fma(u, hu_u, fma(Q, t2, fma(P, t1, -1.0)));
   const double A = HP + HP;                                // dH_orb/dp = A p + B r
-  const double B = (HQ + HQ) * (rp * u2);                  // dH_orb/dr = B p + Cc r
-  const double Cc = -u2 * fma(Hu, u, (HQ + HQ) * Q);
+  const double B = HQ2 * w;                                // dH_orb/dr = B p + Cc r
+  const double Cc = -u2 * fma(Hu, u, HQ2 * Q);
 
   // spin couplings
   const double a1 = dot3(s1, r), a2 = dot3(s2, r), d12 = dot3(s1, s2);
@@ -108,22 +108,22 @@ __device__ __forceinline__ void pn_eval(const C& c, const double* z, double* g, 
   const double LS = dot3(L, Sg);                                      // = H_SO
   const double a12u5 = a1 * a2 * u5;
   const double c12u3 = c[K_C12] * u3;
-  // coefficient of r in dH_spin/dr, in units of u^2:  -3 H_SO + c12 (3 d12 u^3 - 15 a1 a2 u^5) + QM
-  double wr = fma(c12u3, 3.0 * d12, fma(-15.0 * c[K_C12], a12u5, -3.0 * LS));
-  const double c12u5x3 = 3.0 * c[K_C12] * u5;
+  // coefficient of r in dH_spin/dr is 3 u^2 X:  X = -H_SO + c12 (d12 u^3 - 5 a1 a2 u^5) + QM
+  double X = fma(c12u3, d12, fma(c[K_M5C12], a12u5, -LS));
+  const double c12u5x3 = c[K_3C12] * u5;
   double w1 = c12u5x3 * a2, w2 = c12u5x3 * a1;
-  double Hss = fma(3.0 * c[K_C12], a12u5, -(c12u3 * d12));
+  double Hss = fma(c[K_3C12], a12u5, -(c12u3 * d12));
   if (QM) {
     const double d11 = dot3(s1, s1), d22 = dot3(s2, s2);
     const double q1u3 = c[K_Q1] * u3, q2u3 = c[K_Q2] * u3;
     const double a11u5 = a1 * a1 * u5, a22u5 = a2 * a2 * u5;
-    wr = fma(q1u3, 3.0 * d11, fma(-15.0 * c[K_Q1], a11u5, wr));
-    wr = fma(q2u3, 3.0 * d22, fma(-15.0 * c[K_Q2], a22u5, wr));
+    X = fma(q1u3, d11, fma(-5.0 * c[K_Q1], a11u5, X));
+    X = fma(q2u3, d22, fma(-5.0 * c[K_Q2], a22u5, X));
     w1 = fma(6.0 * c[K_Q1] * u5, a1, w1);
     w2 = fma(6.0 * c[K_Q2] * u5, a2, w2);
     Hss += fma(3.0 * c[K_Q1], a11u5, -(q1u3 * d11)) + fma(3.0 * c[K_Q2], a22u5, -(q2u3 * d22));
   }
-  const double Cr = fma(wr, u2, Cc);
+  const double Cr = fma(X, 3.0 * u2, Cc);
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
     g[i] = fma(w2, s2[i], fma(w1, s1[i], fma(Cr, r[i], fma(B, p[i], PxS[i]))));
@@ -132,10 +132,10 @@ __device__ __forceinline__ void pn_eval(const C& c, const double* z, double* g, 
   if (OMEGA) {
     const double o1u = c[K_O1] * u3, o2u = c[K_O2] * u3;
     const double m12u = c[K_M12] * u3, m21u = c[K_M21] * u3;
-    double b1r = c[K_M12] * a2, b2r = c[K_M21] * a1;
-    if (QM) { b1r = fma(c[K_M11], a1, b1r); b2r = fma(c[K_M22], a2, b2r); }
-    b1r *= 3.0 * u5;
-    b2r *= 3.0 * u5;
+    double b1r = c[K_3M12] * a2, b2r = c[K_3M21] * a1;
+    if (QM) { b1r = fma(3.0 * c[K_M11], a1, b1r); b2r = fma(3.0 * c[K_M22], a2, b2r); }
+    b1r *= u5;
+    b2r *= u5;
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
       g[6 + i] = fma(-m12u, s2[i], fma(b1r, r[i], o1u * L[i]));

@@ -48,7 +48,10 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="mc", choices=["mc", "reference"])
     ap.add_argument("--grid", type=int, default=314, help="grid edge (314 = BASELINE config 2)")
-    ap.add_argument("--n-steps", type=int, default=100_000, help="RK4 steps per orbit (1e5 = config 2)")
+    ap.add_argument("--n-steps", type=int, default=None, help="RK4 steps per orbit (default: the workload's own; 1e5 for config 2)")
+    ap.add_argument("--workload", default="config2",
+                    help="config2 (default, the bench line) | config0 | config1 | config1:mode0 | config3 | config3:qmoff | "
+                         "config4:<log2 n>  -- the other BASELINE configs, for profiles/ tables only")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -102,12 +105,40 @@ class ClockSampler(threading.Thread):
 
 
 def global_workload(args, world):
-    """Config 2 widened to 314*world rows of r0 (same r0 range, same theta axis)."""
-    return workloads.config2(n_r=args.grid * world, n_theta=args.grid, n_steps=args.n_steps)
+    """Config 2 widened to 314*world rows of r0 (same r0 range, same theta axis); the other configs are
+    replicated per rank as they are."""
+    name, _, opt = args.workload.partition(":")
+    kw = {} if args.n_steps is None else {"n_steps": args.n_steps}
+    if name == "config2":
+        return workloads.config2(n_r=args.grid * world, n_theta=args.grid, **kw)
+    if name == "config0":
+        return workloads.config0(**kw)
+    if name == "config1":
+        w = workloads.config1(**kw)
+        if opt == "mode0":
+            w.correction_mode = 0
+        return w
+    if name == "config3":
+        return workloads.config3(qm=(opt != "qmoff"), **kw)
+    if name == "config4":
+        return workloads.config4(int(opt or 12), **kw)
+    raise SystemExit(f"unknown workload {args.workload}")
 
 
 def rank_shard(w, args, rank, world):
+    if args.workload.partition(":")[0] != "config2":
+        return w
     return sharding.rank_shard(w, args.grid, args.grid, rank, world)
+
+
+def describe(w, args):
+    if w.name.startswith("config2"):
+        return (f"config2: {args.grid}x{args.grid} orbit scan per GPU (r0 in [10,60] x theta in [0,pi]), equal mass, chi=1, "
+                f"N+1PN+2PN+SO+SS, RK4 h=1, {w.n_steps} steps, shadow 1e-8 renormalised every 100 steps + FLI, "
+                "six-integral correction (mode 3, Gauss-Newton terminated at eps=1e-10, cap 4)")
+    return (f"{args.workload} ({w.name}): {w.n_orbits} orbits per GPU, terms mask {w.terms}, "
+            f"{'uniform' if w.uniform else 'per-orbit'} parameters, RK4 h={w.h}, {w.n_steps} steps, shadow {w.shadow_eps}, "
+            f"correction mode {w.correction_mode}")
 
 
 def cpu_baseline_sample(w, target_seconds=15.0):
@@ -193,7 +224,11 @@ def run_mc(args):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
 
     peak_tf, peak_clock = binding.fp64_peak(local, 200.0) if rank == 0 else (None, None)
-    I = binding.Integrator(terms=w.terms, device=local)
+    if w.uniform:
+        par = dict(beta=float(w.beta[0]), chi1=float(w.chi1[0]), chi2=float(w.chi2[0]), kq1=float(w.kq1[0]), kq2=float(w.kq2[0]))
+    else:
+        par = {k: v for k, v in w.params().items() if k != "terms"}
+    I = binding.Integrator(terms=w.terms, device=local, **par)
     out = torch.empty_like(z_dev)
     stream = torch.cuda.current_stream(dev)
     launches = 0
@@ -241,7 +276,7 @@ def run_mc(args):
 
     info = I.launch_info()
     status = res.status.cpu().numpy()
-    fli = res.fli.cpu().numpy()
+    fli = res.fli.cpu().numpy() if res.fli is not None else np.zeros(n)
     steps_done = float(res.steps_done.sum().item())          # accepted orbit-steps of one launch (this rank)
     gn_steps = float(I.work(n).sum().item())                  # Gauss-Newton steps of one launch, orbit + shadow
     steps_done_job = sharding.sum_over_ranks(steps_done, dev)
@@ -262,7 +297,7 @@ def run_mc(args):
     achieved_tf = flop_per_launch / per_launch_s / 1e12
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": nominal_tf, "unit": "TFLOP/s",
                 "frac": achieved_tf / nominal_tf,
-                "traffic": NCU_DRAM_BYTES_PER_LAUNCH_314 if (args.grid == 314 and world == 1) else None,
+                "traffic": NCU_DRAM_BYTES_PER_LAUNCH_314 if (w.name.startswith("config2") and args.grid == 314 and world == 1) else None,
                 "traffic_unit": "bytes per launch (ncu capture, profiles/r01b_ncu_integrate_kernel_mode3.md)",
                 "algorithmic_bytes_per_launch": 340.0 * n,
                 "peak_source": f"derived: {info['num_sms']} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x {sm_max:.0f} MHz "
@@ -271,16 +306,14 @@ def run_mc(args):
                 "dfma_probe_implied_sm_mhz": peak_clock,
                 "flop_per_launch": flop_per_launch, "flop_per_orbit_step": flop_per_launch / max(steps_done, 1.0),
                 "gn_steps_per_trajectory_step": gn_steps / max(2.0 * steps_done, 1.0),
-                "accepted_orbit_steps_per_launch": steps_done, "kernel": "mc::integrate_kernel<uniform,QM off,mode 3>",
+                "accepted_orbit_steps_per_launch": steps_done, "kernel": "mc::integrate_kernel<%s,QM %s,mode %d>" % ("uniform" if w.uniform else "per-orbit", "on" if w.terms & 16 else "off", w.correction_mode),
                 "kernel_ms_per_launch": dev_ms / args.steps,
                 "regs_per_thread": info["regs_per_thread"], "spill_bytes": info["local_bytes"],
                 "blocks_per_sm": info["blocks_per_sm"], "grid": info["grid"], "block": info["block"]}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"config2: {args.grid}x{args.grid} orbit scan per GPU (r0 in [10,60] x theta in [0,pi]), "
-                                   f"equal mass, chi=1, N+1PN+2PN+SO+SS, RK4 h=1, {w.n_steps} steps, shadow 1e-8 "
-                                   "renormalised every 100 steps + FLI, six-integral correction (mode 3, Gauss-Newton terminated at eps=1e-10, cap 4)",
+            "config": {"workload": describe(w, args),
                        "orbits_per_gpu": n, "rk4_steps": w.n_steps,
                        "orbit_steps_counted": "accepted steps (sum of steps_done); scheduled = orbits x rk4_steps = %d" % int(orbit_steps_rank * world), "l2": "flushed (256 MiB write) between timed iterations",
                        "parallelism": f"orbit-sharded x{world}, no collective"},

@@ -51,7 +51,8 @@ def parse_args():
     ap.add_argument("--n-steps", type=int, default=None, help="RK4 steps per orbit (default: the workload's own; 1e5 for config 2)")
     ap.add_argument("--workload", default="config2",
                     help="config2 (default, the bench line) | config0 | config1 | config1:mode0 | config3 | config3:qmoff | "
-                         "config4:<log2 n>  -- the other BASELINE configs, for profiles/ tables only")
+                         "config4:<log2 n> | paper-theta2 | paper-theta2:0 | paper-plane  -- the other BASELINE configs and the "
+                         "paper's own scans (PAPER.md:227), for profiles/ tables only")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -122,6 +123,10 @@ def global_workload(args, world):
         return workloads.config3(qm=(opt != "qmoff"), **kw)
     if name == "config4":
         return workloads.config4(int(opt or 12), **kw)
+    if name == "paper-theta2":                      # PAPER.md:227, Fig 6a (theta1 = pi/2) / 6b (paper-theta2:0)
+        return workloads.paper_scan_theta2(theta1=(0.0 if opt == "0" else np.pi / 2), **kw)
+    if name == "paper-plane":                       # PAPER.md:227, Fig 7
+        return workloads.paper_scan_plane(**kw)
     raise SystemExit(f"unknown workload {args.workload}")
 
 

@@ -144,6 +144,40 @@ def config4(log2_n=12, n_steps=20_000):
                     _full(n, 1), _full(n, 1), n_steps=n_steps, shadow_eps=1e-8)
 
 
+def _spin_xz(theta):
+    """Unit vector at angle theta from +z in the x-z plane: (sin theta, 0, cos theta)."""
+    theta = np.asarray(theta, dtype=np.float64)
+    return np.stack([np.sin(theta), np.zeros_like(theta), np.cos(theta)])
+
+
+def paper_scan_theta2(theta1=np.pi / 2, n=314, dtheta=0.01, n_steps=100_000):
+    """The paper's 1-D scan (Fig 6): beta = 1/3, r = (5.65,0,0), p = (0,0.765,0), chi = 1,
+    theta1 fixed (pi/2 for Fig 6a, 0 for Fig 6b), theta2 = 0, 0.01, ..., 3.13 (314 orbits), t = 1e5, FLI."""
+    th2 = dtheta * np.arange(n)
+    z = np.zeros((12, n))
+    z[0] = 5.65
+    z[4] = 0.765
+    z[6:9] = _spin_xz(np.full(n, theta1))
+    z[9:12] = _spin_xz(th2)
+    return Workload(f"paper-scan-theta2(theta1={theta1:.4f})", z, _full(n, 1.0 / 3.0), _full(n, 1), _full(n, 1),
+                    _full(n, 1), _full(n, 1), n_steps=n_steps, shadow_eps=1e-8, meta=dict(theta2=th2))
+
+
+def paper_scan_plane(n1=314, n2=314, dtheta=0.01, n_steps=100_000):
+    """The paper's 2-D scan (Fig 7): (theta1, theta2) plane, 314 x 314 orbits, r = (10.14,0,0),
+    p = (0,0.365,0) (orbit 2's initial state, hence beta = 1; R20), chi = 1.  Index = i1*n2 + i2."""
+    T1, T2 = np.meshgrid(dtheta * np.arange(n1), dtheta * np.arange(n2), indexing="ij")
+    T1, T2 = T1.ravel(), T2.ravel()
+    n = T1.size
+    z = np.zeros((12, n))
+    z[0] = 10.14
+    z[4] = 0.365
+    z[6:9] = _spin_xz(T1)
+    z[9:12] = _spin_xz(T2)
+    return Workload("paper-scan-plane", z, _full(n, 1), _full(n, 1), _full(n, 1), _full(n, 1), _full(n, 1),
+                    n_steps=n_steps, shadow_eps=1e-8, meta=dict(shape=(n1, n2), theta1=T1, theta2=T2))
+
+
 def shard_range(n_units: int, rank: int, world_size: int):
     """Contiguous, balanced [lo, hi) range of orbit indices owned by `rank` (no collective needed)."""
     base, rem = divmod(n_units, world_size)

@@ -336,3 +336,28 @@ def test_classification_agreement_at_1e5_steps_on_a_strided_subgrid(mc):
     assert ((cg == 2) == (co == 2)).mean() >= 0.995                                       # dropped cells
     reg = (co == 0) & (o.fli < 4.5) & (cg == 0)
     assert np.abs(gfli[idx][reg] - o.fli[reg]).max() < 0.1
+
+
+@pytest.mark.parametrize("which", ["theta2", "theta2-0", "plane"])
+def test_papers_own_scans_match_oracle(mc, which):
+    """the paper's scans (Figs 6-7) -- beta = 1/3 at r = 5.65 (strong field) and
+    the (theta1, theta2) plane at r = 10.14.  All 314 orbits of the 1-D scans / a 13 x 13 sub-plane, 2000 steps."""
+    if which == "plane":
+        w = workloads.paper_scan_plane(13, 13, dtheta=0.26)
+        par = dict(beta=1.0)
+    else:
+        w = workloads.paper_scan_theta2(theta1=0.0 if which == "theta2-0" else np.pi / 2)
+        par = dict(beta=1.0 / 3.0)
+    with mc.Integrator(**par) as I:
+        g = I.integrate(w.states, 1.0, 2000, 3, shadow_eps=1e-8)
+    o = oracle.integrate(w.states, 1.0, 2000, 3, shadow_eps=1e-8, **w.params())
+    gs, gz, gfli = g.status.cpu().numpy(), g.states.cpu().numpy(), g.fli.cpu().numpy()
+    assert np.array_equal(gs, o.status)
+    assert np.array_equal(g.steps_done.cpu().numpy(), o.steps_done)
+    live = o.status == 0
+    assert live.sum() >= 0.5 * w.n_orbits
+    assert drift(gz[:, live], o.invariants[0:6][:, live], **w.subset(np.where(live)[0]).params()) <= DRIFT_TOL
+    calm = live & (o.fli < 3.0)                        # short-time regular cells: values agree
+    assert calm.sum() >= 0.3 * w.n_orbits
+    assert np.abs(gfli[calm] - o.fli[calm]).max() < 1e-2
+    assert rel_state_err(gz[:, calm], o.states[:, calm]) < 1e-7

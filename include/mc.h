@@ -79,10 +79,14 @@ typedef struct mc_params {
   double r_merge;          /* default 2    (R13)                                                 */
   double r_escape;         /* default 1e4                                                                  */
   void* cuda_stream;       /* cudaStream_t all work is enqueued on (e.g. torch's current stream); NULL = 0 */
+  int32_t chunk_steps;     /* scheduling only, never changes a result bit: 0 = automatic; > 0 = the kernel's
+                              work items are chunks of this many steps (state parked in device scratch owned
+                              by the handle between chunks)                          */
 } mc_params;
 
 /* Fill *p with defaults: terms = 1PN|2PN|SO|S1S2, device 0, uniform beta = chi = kq = 1,
- * renorm_interval 100, newton_iters 4, newton_tol 1e-10, r_merge 2, r_escape 1e4, stream NULL. */
+ * renorm_interval 100, newton_iters 4, newton_tol 1e-10, r_merge 2, r_escape 1e4, stream NULL,
+ * chunk_steps 0. */
 int mc_params_default(mc_params* p);
 
 /* Validate params, select the device, allocate the handle.  *out_handle is set only on success. */
@@ -103,8 +107,8 @@ int mc_create(const mc_params* params, mc_handle** out_handle);
  *                   the (normalised) input state, rows 6-11 = the same of the output state
  *   out_fli         DEVICE, double[n_orbits]; required iff shadow_eps != 0
  *
- * The call is asynchronous on params.cuda_stream: one kernel launch, no host synchronisation, no
- * host<->device copy.  All buffers are owned by the caller.  n_orbits = 0 or n_steps = 0 are valid
+ * The call is asynchronous on params.cuda_stream: one kernel launch (preceded by one memset of the
+ * work-queue scratch), no host synchronisation, no host<->device copy.  All buffers are owned by the caller.  n_orbits = 0 or n_steps = 0 are valid
  * (n_steps = 0 copies the normalised state and evaluates the invariants).  Numerical failures of
  * single orbits are not errors: see mc_get_status.
  * Errors: MC_EINVAL (null/negative arguments, n_steps >= 2^31, unknown mode, non-finite step_h), MC_ECUDA. */
@@ -151,6 +155,8 @@ typedef struct mc_launch_info {
   int32_t smem_bytes;           /* dynamic shared memory per block                */
   int32_t variant;              /* bit0 per-orbit params, bit1 QM, bits 4-5 mode  */
   int64_t trajectories;         /* threads doing work = n_orbits * (1 + shadow)   */
+  int32_t chunk_steps;          /* steps per work item                             */
+  int32_t n_chunks;             /* work items per 32-trajectory unit              */
 } mc_launch_info;
 int mc_last_launch_info(mc_handle* h, mc_launch_info* out);
 

@@ -37,13 +37,14 @@ class mc_params(ctypes.Structure):
                 ("d_beta", ctypes.c_void_p), ("d_chi1", ctypes.c_void_p), ("d_chi2", ctypes.c_void_p),
                 ("d_kq1", ctypes.c_void_p), ("d_kq2", ctypes.c_void_p), ("renorm_interval", ctypes.c_int32),
                 ("newton_iters", ctypes.c_int32), ("newton_tol", ctypes.c_double), ("r_merge", ctypes.c_double),
-                ("r_escape", ctypes.c_double), ("cuda_stream", ctypes.c_void_p)]
+                ("r_escape", ctypes.c_double), ("cuda_stream", ctypes.c_void_p), ("chunk_steps", ctypes.c_int32)]
 
 
 class mc_launch_info(ctypes.Structure):
     _fields_ = [("grid", ctypes.c_int32), ("block", ctypes.c_int32), ("regs_per_thread", ctypes.c_int32),
                 ("local_bytes", ctypes.c_int32), ("blocks_per_sm", ctypes.c_int32), ("num_sms", ctypes.c_int32),
-                ("smem_bytes", ctypes.c_int32), ("variant", ctypes.c_int32), ("trajectories", ctypes.c_int64)]
+                ("smem_bytes", ctypes.c_int32), ("variant", ctypes.c_int32), ("trajectories", ctypes.c_int64),
+                ("chunk_steps", ctypes.c_int32), ("n_chunks", ctypes.c_int32)]
 
 
 _lib = None
@@ -121,7 +122,8 @@ class Integrator:
     """mc_create / mc_integrate / mc_destroy with torch tensors as device buffers."""
 
     def __init__(self, terms=TERMS_DEFAULT, beta=1.0, chi1=1.0, chi2=1.0, kq1=1.0, kq2=1.0, device=0,
-                 renorm_interval=100, newton_iters=4, newton_tol=1e-10, r_merge=2.0, r_escape=1e4, stream=None):
+                 renorm_interval=100, newton_iters=4, newton_tol=1e-10, r_merge=2.0, r_escape=1e4, stream=None,
+                 chunk_steps=0):
         import torch
         self._torch = torch
         self._lib = load_library()
@@ -129,6 +131,7 @@ class Integrator:
         p.terms, p.device = int(terms), int(device)
         p.renorm_interval, p.newton_iters, p.newton_tol = int(renorm_interval), int(newton_iters), float(newton_tol)
         p.r_merge, p.r_escape = float(r_merge), float(r_escape)
+        p.chunk_steps = int(chunk_steps)
         self.device = torch.device("cuda", device)
         vals = dict(beta=beta, chi1=chi1, chi2=chi2, kq1=kq1, kq2=kq2)
         per_orbit = any(hasattr(v, "__len__") for v in vals.values())

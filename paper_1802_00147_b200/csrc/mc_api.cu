@@ -55,6 +55,7 @@ struct mc_handle {
   int num_sms;
   int64_t last_n;            // orbits of the last mc_integrate (status buffers valid for these)
   DeviceBuf status, step, gn;   // int32[n], int64[n], int64[n]
+  DeviceBuf sched, carry_d, carry_i, carry_g;   // work queue + per-unit flags; carried state between chunks
   DeviceBuf h_in, h_out, h_inv, h_fli;   // scratch of mc_integrate_host
   mc_launch_info info;
 };
@@ -168,6 +169,7 @@ int mc_params_default(mc_params* p) {
   p->r_merge = 2.0;
   p->r_escape = 1e4;
   p->cuda_stream = nullptr;
+  p->chunk_steps = 0;
   return MC_OK;
 }
 
@@ -176,6 +178,7 @@ int mc_create(const mc_params* params, mc_handle** out_handle) {
   if (params->struct_size != sizeof(mc_params)) return MC_EINVAL;
   if (params->terms & ~31u) return MC_EINVAL;
   if (params->renorm_interval <= 0 || params->newton_iters < 1 || params->newton_iters > 16) return MC_EINVAL;
+  if (params->chunk_steps < 0) return MC_EINVAL;
   if (!(params->newton_tol >= 0.0) || !(params->r_merge >= 0.0) || !(params->r_escape > params->r_merge)) return MC_EINVAL;
   if (params->per_orbit) {
     if (!params->d_beta || !params->d_chi1 || !params->d_chi2 || !params->d_kq1 || !params->d_kq2) return MC_EINVAL;
@@ -236,11 +239,45 @@ int mc_integrate(mc_handle* h, const double* states, int64_t n_orbits, double st
     default: fn = mc::launcher_mode3(h->P.per_orbit != 0, qm); break;
   }
   const int64_t traj = n_orbits * (shadow ? 2 : 1);
-  const int64_t grid = (traj + mc::kBlock - 1) / mc::kBlock;
-  if (grid > 0x7fffffffLL) return MC_EINVAL;
+  A.n_units = (traj + 31) / 32;
+  if (A.n_units > 0x3fffffffLL) return MC_EINVAL;
+  A.chunk_len = 1; A.n_chunks = 1; A.n_items = A.n_units;
   mc::KernelInfo ki;
-  MC_CUDA(fn(h->uc, A, (int)grid, h->stream, &ki));
-  h->info.grid = (int32_t)grid;
+  MC_CUDA(fn(h->uc, A, h->num_sms, false, h->stream, &ki));                  // occupancy / register query
+  // Chunking policy: one chunk when every unit is resident at once (nothing to balance)
+  // or the run is short; otherwise about 128 chunks of >= 256 steps, a multiple of renorm_interval.
+  const int64_t slots = (int64_t)h->num_sms * ki.blocks_per_sm * (mc::kBlock / 32);
+  int64_t chunk = n_steps > 0 ? n_steps : 1;
+  if (h->P.chunk_steps > 0) {
+    chunk = h->P.chunk_steps;
+  } else if (A.n_units > slots && n_steps >= 512) {
+    chunk = (n_steps + 127) / 128;
+    if (chunk < 256) chunk = 256;
+    const int64_t ri = h->P.renorm_interval;
+    if (shadow) chunk = ((chunk + ri - 1) / ri) * ri;
+  }
+  if (chunk > 0x7fffffffLL) chunk = 0x7fffffffLL;
+  int64_t n_chunks = n_steps > 0 ? (n_steps + chunk - 1) / chunk : 1;
+  if (n_chunks > 0x7fffffffLL) return MC_EINVAL;
+  A.chunk_len = (int32_t)chunk;
+  A.n_chunks = (int32_t)n_chunks;
+  A.n_items = A.n_units * n_chunks;
+  rc = h->sched.reserve(16 + sizeof(int32_t) * (size_t)A.n_units);
+  if (rc) return rc;
+  A.queue = (unsigned long long*)h->sched.p;
+  A.done = (int32_t*)((char*)h->sched.p + 16);
+  if (n_chunks > 1) {
+    const size_t tp = (size_t)A.n_units * 32;
+    if ((rc = h->carry_d.reserve(sizeof(double) * 17 * tp))) return rc;
+    if ((rc = h->carry_i.reserve(sizeof(int32_t) * 3 * tp))) return rc;
+    if ((rc = h->carry_g.reserve(sizeof(unsigned long long) * tp))) return rc;
+    A.carry_d = (double*)h->carry_d.p; A.carry_i = (int32_t*)h->carry_i.p; A.carry_g = (unsigned long long*)h->carry_g.p;
+  }
+  MC_CUDA(cudaMemsetAsync(h->sched.p, 0, 16 + sizeof(int32_t) * (size_t)A.n_units, h->stream));
+  MC_CUDA(fn(h->uc, A, h->num_sms, true, h->stream, &ki));
+  h->info.grid = ki.grid;
+  h->info.chunk_steps = A.chunk_len;
+  h->info.n_chunks = A.n_chunks;
   h->info.block = ki.block;
   h->info.regs_per_thread = ki.regs;
   h->info.local_bytes = ki.local_bytes;
@@ -366,6 +403,7 @@ int mc_destroy(mc_handle* h) {
   if (!h) return MC_EINVAL;
   cudaSetDevice(h->P.device);
   h->status.release(); h->step.release(); h->gn.release();
+  h->sched.release(); h->carry_d.release(); h->carry_i.release(); h->carry_g.release();
   h->h_in.release(); h->h_out.release(); h->h_inv.release(); h->h_fli.release();
   delete h;
   return MC_OK;

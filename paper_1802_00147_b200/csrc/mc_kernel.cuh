@@ -1,7 +1,15 @@
-// mc_kernel.cuh -- the integration kernel: one thread per trajectory, whole state in registers for
-// all n_steps; with a shadow, lanes (2k, 2k+1) of a warp hold orbit k's main and shadow trajectory and
+// mc_kernel.cuh -- the integration kernel: one thread per trajectory, whole state in registers inside
+// the step loop; with a shadow, lanes (2k, 2k+1) of a warp hold orbit k's main and shadow trajectory and
 // meet through warp shuffles (status every step, distance every renorm_interval steps).
-// Global memory is touched at launch (coalesced SoA loads) and at the end (coalesced SoA stores) only.
+//
+// Scheduling: the grid is persistent (as many blocks as are resident at once) and
+// every WARP pulls work items from a global queue.  An item is (chunk c, unit u): unit u = 32 consecutive
+// trajectories, chunk c = steps [c*chunk_len, (c+1)*chunk_len).  Items are numbered chunk-major, so unit
+// u's chunk c+1 is handed out n_units items after its chunk c; between chunks the trajectory state
+// (17 doubles + 20 bytes) rests in an L2-resident carry buffer and a per-unit flag publishes it.  When
+// everything is resident at once there is one chunk and no carry traffic.  Otherwise the chunks remove
+// the partial last wave: all SMs stay busy until the last chunk.
+// Global memory is touched at launch, at chunk boundaries and at the end only, always coalesced SoA.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -28,6 +36,16 @@ struct IntegrateArgs {
   uint32_t terms;
   int32_t renorm_interval;
   int32_t newton_iters;
+  // scheduling
+  unsigned long long* queue;  // [0] = next item
+  int32_t* done;              // [n_units] chunks completed per unit
+  double* carry_d;            // [17][n_traj_padded]: y[12], E0, J0[3], acc
+  int32_t* carry_i;           // [3][n_traj_padded]: status | flag << 16 | frozen << 31, steps, until_renorm
+  unsigned long long* carry_g;  // [n_traj_padded]: Gauss-Newton steps
+  int64_t n_units;            // ceil(trajectories / 32)
+  int64_t n_items;            // n_units * n_chunks
+  int32_t chunk_len;          // steps per chunk (>= 1)
+  int32_t n_chunks;
 };
 
 enum { ST_OK = 0, ST_MERGED = 1, ST_UNBOUND = 2, ST_NONFINITE = 3, ST_NEWTON_FLAG = 256 };
@@ -58,129 +76,188 @@ __global__ void MC_KERNEL_BOUNDS(MINB)
 integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ IntegrateArgs A) {
   extern __shared__ double smem[];   // PER_ORBIT: [MC_NCONST][kBlock]
   const bool shadow = A.shadow_eps != 0.0;
-  const int64_t t = (int64_t)blockIdx.x * kBlock + threadIdx.x;
-  const int64_t orbit_raw = shadow ? (t >> 1) : t;
-  const bool role_shadow = shadow && (t & 1);
-  const bool active = orbit_raw < A.n;
-  const int64_t orbit = active ? orbit_raw : (A.n - 1);   // idle lanes shadow-compute a valid orbit, never store
-
-  using CP = typename std::conditional<PER_ORBIT, SharedConsts, UniformConsts>::type;
-  CP c = [&]() {
-    if constexpr (PER_ORBIT) {
-      mc_derive_consts(A.beta[orbit], A.chi1[orbit], A.chi2[orbit], A.kq1[orbit], A.kq2[orbit], A.terms,
-                       smem + threadIdx.x, kBlock);
-      return SharedConsts{smem + threadIdx.x, kBlock};
-    } else {
-      return UniformConsts{uc};
-    }
-  }();
-
-  double y[12];
-#pragma unroll
-  for (int i = 0; i < 12; ++i) y[i] = A.states[(int64_t)i * A.n + orbit];
-  if (MODE >= 1) { normalise3(y + 6); normalise3(y + 9); }
-  if (!role_shadow && active && A.out_inv) {   // rows 0-5: the main trajectory before the offset; stored now so
-    double inv0[6];                            // that nothing of it stays in registers during the step loop
-    six_integrals<QM>(c, y, inv0);
-#pragma unroll
-    for (int i = 0; i < 6; ++i) A.out_inv[(int64_t)i * A.n + orbit] = inv0[i];
-  }
+  const int lane = threadIdx.x & 31;
+  const int64_t tp = A.n_units * 32;   // padded trajectory count = stride of the carry arrays
   const double d0 = fabs(A.shadow_eps);
-  if (role_shadow) y[0] += A.shadow_eps;
-  Refs R;
-  references<QM>(c, y, R);
+  const int n_steps = (int)A.n_steps;  // < 2^31 (mc_integrate checks)
 
-  int status = ST_OK, flag = 0;
-  bool frozen = false;
-  int steps = 0;            // n_steps < 2^31 (mc_integrate checks)
-  unsigned long long gn_total = 0;
-  double acc = 0.0;
-  int until_renorm = A.renorm_interval;
-
-  const int n_steps = (int)A.n_steps;
 #pragma unroll 1
-  for (int k = 0; k < n_steps; ++k) {
-    double z[12];
-    rk4_step<QM>(c, y, A.h, z);
-    int gn;
-    const bool ok = correct<MODE, QM>(c, z, R, A.newton_iters, A.newton_tol, gn);
-    if (MODE == 2 && !ok && !role_shadow && !frozen) flag = ST_NEWTON_FLAG;
-    // status of the completed step (R13): non-finite anywhere in the pair, else |r| of the main
-    int code = ST_OK;
-    if (!finite12(z)) code = ST_NONFINITE;
-    else if (!role_shadow) {
-      const double r2 = dot3(z, z);
-      code = (r2 < A.r_merge2) ? ST_MERGED : ((r2 > A.r_escape2) ? ST_UNBOUND : ST_OK);
-    }
-    if (shadow) {
-      const int other = __shfl_xor_sync(0xffffffffu, code, 1);
-      code = (code == ST_NONFINITE || other == ST_NONFINITE) ? ST_NONFINITE : (role_shadow ? other : code);
-    }
-    if (!frozen) {
-      if (code == ST_OK) {
-#pragma unroll
-        for (int i = 0; i < 12; ++i) y[i] = z[i];
-        ++steps;
-        gn_total += (unsigned)gn;
+  for (;;) {
+    unsigned long long item = 0;
+    if (lane == 0) item = atomicAdd(A.queue, 1ULL);
+    item = __shfl_sync(0xffffffffu, item, 0);
+    if (item >= (unsigned long long)A.n_items) break;
+    const int chunk = (int)(item / (unsigned long long)A.n_units);
+    const int64_t unit = (int64_t)(item % (unsigned long long)A.n_units);
+    const int64_t t = unit * 32 + lane;
+    const int64_t orbit_raw = shadow ? (t >> 1) : t;
+    const bool role_shadow = shadow && (t & 1);
+    const bool active = orbit_raw < A.n;
+    const int64_t orbit = active ? orbit_raw : (A.n - 1);   // idle lanes shadow-compute a valid orbit, never store
+
+    using CP = typename std::conditional<PER_ORBIT, SharedConsts, UniformConsts>::type;
+    CP c = [&]() {
+      if constexpr (PER_ORBIT) {
+        mc_derive_consts(A.beta[orbit], A.chi1[orbit], A.chi2[orbit], A.kq1[orbit], A.kq2[orbit], A.terms,
+                         smem + threadIdx.x, kBlock);
+        return SharedConsts{smem + threadIdx.x, kBlock};
       } else {
-        frozen = true;
-        status = code;
+        return UniformConsts{uc};
+      }
+    }();
+
+    double y[12];
+    Refs R;
+    int status = ST_OK, flag = 0;
+    bool frozen = false;
+    int steps = 0;
+    unsigned long long gn_total = 0;
+    double acc = 0.0;
+    int until_renorm = A.renorm_interval;
+
+    if (chunk == 0) {
+      // prologue: coalesced SoA load, eq (10) on the input, reference integrals
+#pragma unroll
+      for (int i = 0; i < 12; ++i) y[i] = A.states[(int64_t)i * A.n + orbit];
+      if (MODE >= 1) { normalise3(y + 6); normalise3(y + 9); }
+      if (!role_shadow && active && A.out_inv) {   // rows 0-5: the main trajectory before the offset
+        double inv0[6];
+        six_integrals<QM>(c, y, inv0);
+#pragma unroll
+        for (int i = 0; i < 6; ++i) A.out_inv[(int64_t)i * A.n + orbit] = inv0[i];
+      }
+      if (role_shadow) y[0] += A.shadow_eps;
+      references<QM>(c, y, R);
+    } else {
+      // wait until this unit's previous chunk is published, then reload the carried state.  The holder of
+      // that chunk got it earlier from the same queue, so it is running: the wait cannot deadlock.
+      if (lane == 0) {
+        unsigned polls = 0;
+        while (*(volatile int32_t*)(A.done + unit) < chunk) {
+          __nanosleep(100);
+          if (++polls > (1u << 27)) __trap();   // > 10 s: something is broken, fail loudly instead of hanging
+        }
+      }
+      __syncwarp();
+      __threadfence();
+#pragma unroll
+      for (int i = 0; i < 12; ++i) y[i] = __ldcg(A.carry_d + (int64_t)i * tp + t);   // L2 only: L1 may be stale
+      R.E0 = __ldcg(A.carry_d + 12 * tp + t);
+#pragma unroll
+      for (int i = 0; i < 3; ++i) R.J0[i] = __ldcg(A.carry_d + (int64_t)(13 + i) * tp + t);
+      acc = __ldcg(A.carry_d + 16 * tp + t);
+      const int packed = __ldcg(A.carry_i + t);
+      status = packed & 0xff;
+      flag = (packed >> 8) & ST_NEWTON_FLAG;   // bit 16 -> 256
+      frozen = packed < 0;
+      steps = __ldcg(A.carry_i + tp + t);
+      until_renorm = __ldcg(A.carry_i + 2 * tp + t);
+      gn_total = __ldcg(A.carry_g + t);
+    }
+
+    const int k_end = min(n_steps, (chunk + 1 == A.n_chunks) ? n_steps : (chunk + 1) * A.chunk_len);
+#pragma unroll 1
+    for (int k = chunk * A.chunk_len; k < k_end; ++k) {
+      if (__all_sync(0xffffffffu, frozen)) break;
+      double z[12];
+      rk4_step<QM>(c, y, A.h, z);
+      int gn;
+      const bool ok = correct<MODE, QM>(c, z, R, A.newton_iters, A.newton_tol, gn);
+      if (MODE == 2 && !ok && !role_shadow && !frozen) flag = ST_NEWTON_FLAG;
+      // status of the completed step (R13): non-finite anywhere in the pair, else |r| of the main
+      int code = ST_OK;
+      if (!finite12(z)) code = ST_NONFINITE;
+      else if (!role_shadow) {
+        const double r2 = dot3(z, z);
+        code = (r2 < A.r_merge2) ? ST_MERGED : ((r2 > A.r_escape2) ? ST_UNBOUND : ST_OK);
+      }
+      if (shadow) {
+        const int other = __shfl_xor_sync(0xffffffffu, code, 1);
+        code = (code == ST_NONFINITE || other == ST_NONFINITE) ? ST_NONFINITE : (role_shadow ? other : code);
+      }
+      if (!frozen) {
+        if (code == ST_OK) {
+#pragma unroll
+          for (int i = 0; i < 12; ++i) y[i] = z[i];
+          ++steps;
+          gn_total += (unsigned)gn;
+        } else {
+          frozen = true;
+          status = code;
+        }
+      }
+      if (shadow && --until_renorm == 0) {
+        until_renorm = A.renorm_interval;
+        // shadow lane pulls the main state; d = |z' - z| over all 12 components (R10, R12)
+        double ym[12];
+#pragma unroll
+        for (int i = 0; i < 12; ++i) ym[i] = __shfl_xor_sync(0xffffffffu, y[i], 1);
+        int bad = 0;
+        if (role_shadow && !frozen) {
+          double d2 = 0.0;
+#pragma unroll
+          for (int i = 0; i < 12; ++i) { const double e = y[i] - ym[i]; d2 = fma(e, e, d2); }
+          const double d = sqrt(d2);
+          if (!(d > 0.0) || !(d < 1.0e300)) {
+            bad = 1;
+          } else {
+            acc += log10(d / d0);
+            const double s = d0 / d;
+#pragma unroll
+            for (int i = 0; i < 12; ++i) y[i] = fma(s, y[i] - ym[i], ym[i]);
+            if (MODE >= 1) { normalise3(y + 6); normalise3(y + 9); }
+            references<QM>(c, y, R);   // the shadow obeys its own, re-referenced integrals (R11)
+          }
+        }
+        bad |= __shfl_xor_sync(0xffffffffu, bad, 1);
+        if (bad && !frozen) { frozen = true; status = ST_NONFINITE; }
       }
     }
-    if (shadow && --until_renorm == 0) {
-      until_renorm = A.renorm_interval;
-      // shadow lane pulls the main state; d = |z' - z| over all 12 components (R10, R12)
+
+    if (chunk + 1 < A.n_chunks) {
+      // park the state in the carry buffer and publish the chunk
+#pragma unroll
+      for (int i = 0; i < 12; ++i) __stcg(A.carry_d + (int64_t)i * tp + t, y[i]);
+      __stcg(A.carry_d + 12 * tp + t, R.E0);
+#pragma unroll
+      for (int i = 0; i < 3; ++i) __stcg(A.carry_d + (int64_t)(13 + i) * tp + t, R.J0[i]);
+      __stcg(A.carry_d + 16 * tp + t, acc);
+      __stcg(A.carry_i + t, (status & 0xff) | (flag << 8) | (frozen ? (int)0x80000000 : 0));
+      __stcg(A.carry_i + tp + t, steps);
+      __stcg(A.carry_i + 2 * tp + t, until_renorm);
+      __stcg(A.carry_g + t, gn_total);
+      __threadfence();
+      __syncwarp();
+      if (lane == 0) atomicExch(A.done + unit, chunk + 1);
+      continue;
+    }
+
+    // epilogue: FLI from the final separation, invariants, coalesced SoA stores
+    if (shadow) gn_total += __shfl_xor_sync(0xffffffffu, gn_total, 1);
+    if (shadow) {
       double ym[12];
 #pragma unroll
       for (int i = 0; i < 12; ++i) ym[i] = __shfl_xor_sync(0xffffffffu, y[i], 1);
-      int bad = 0;
-      if (role_shadow && !frozen) {
+      if (role_shadow && active) {
         double d2 = 0.0;
 #pragma unroll
         for (int i = 0; i < 12; ++i) { const double e = y[i] - ym[i]; d2 = fma(e, e, d2); }
-        const double d = sqrt(d2);
-        if (!(d > 0.0) || !(d < 1.0e300)) {
-          bad = 1;
-        } else {
-          acc += log10(d / d0);
-          const double s = d0 / d;
-#pragma unroll
-          for (int i = 0; i < 12; ++i) y[i] = fma(s, y[i] - ym[i], ym[i]);
-          if (MODE >= 1) { normalise3(y + 6); normalise3(y + 9); }
-          references<QM>(c, y, R);   // the shadow obeys its own, re-referenced integrals (R11)
-        }
+        A.out_fli[orbit] = acc + log10(sqrt(d2) / d0);
       }
-      bad |= __shfl_xor_sync(0xffffffffu, bad, 1);
-      if (bad && !frozen) { frozen = true; status = ST_NONFINITE; }
     }
-    if (__all_sync(0xffffffffu, frozen)) break;
-  }
-
-  // epilogue: FLI from the final separation, invariants, coalesced SoA stores
-  if (shadow) gn_total += __shfl_xor_sync(0xffffffffu, gn_total, 1);
-  if (shadow) {
-    double ym[12];
+    if (!role_shadow && active) {
 #pragma unroll
-    for (int i = 0; i < 12; ++i) ym[i] = __shfl_xor_sync(0xffffffffu, y[i], 1);
-    if (role_shadow && active) {
-      double d2 = 0.0;
+      for (int i = 0; i < 12; ++i) A.out_states[(int64_t)i * A.n + orbit] = y[i];
+      if (A.out_inv) {
+        double inv1[6];
+        six_integrals<QM>(c, y, inv1);
 #pragma unroll
-      for (int i = 0; i < 12; ++i) { const double e = y[i] - ym[i]; d2 = fma(e, e, d2); }
-      A.out_fli[orbit] = acc + log10(sqrt(d2) / d0);
+        for (int i = 0; i < 6; ++i) A.out_inv[(int64_t)(6 + i) * A.n + orbit] = inv1[i];
+      }
+      A.out_status[orbit] = status | flag;
+      A.out_step[orbit] = steps;
+      A.out_gn[orbit] = (int64_t)gn_total;
     }
-  }
-  if (!role_shadow && active) {
-#pragma unroll
-    for (int i = 0; i < 12; ++i) A.out_states[(int64_t)i * A.n + orbit] = y[i];
-    if (A.out_inv) {
-      double inv1[6];
-      six_integrals<QM>(c, y, inv1);
-#pragma unroll
-      for (int i = 0; i < 6; ++i) A.out_inv[(int64_t)(6 + i) * A.n + orbit] = inv1[i];
-    }
-    A.out_status[orbit] = status | flag;
-    A.out_step[orbit] = steps;
-    A.out_gn[orbit] = (int64_t)gn_total;
   }
 }
 

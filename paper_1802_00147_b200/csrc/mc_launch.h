@@ -7,8 +7,10 @@
 
 namespace mc {
 struct IntegrateArgs;
-struct KernelInfo { int regs, local_bytes, blocks_per_sm, block; size_t smem; };
-typedef cudaError_t (*LaunchFn)(const McConsts&, const IntegrateArgs&, int grid, cudaStream_t, KernelInfo*);
+struct KernelInfo { int regs, local_bytes, blocks_per_sm, block, grid; size_t smem; };
+// query: fills KernelInfo (occupancy, registers) without launching.  launch: starts min(blocks needed,
+// resident capacity) persistent blocks.
+typedef cudaError_t (*LaunchFn)(const McConsts&, const IntegrateArgs&, int num_sms, bool do_launch, cudaStream_t, KernelInfo*);
 LaunchFn launcher_mode0(bool per_orbit, bool qm);
 LaunchFn launcher_mode1(bool per_orbit, bool qm);
 LaunchFn launcher_mode2(bool per_orbit, bool qm);

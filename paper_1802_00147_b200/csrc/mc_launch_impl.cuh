@@ -8,8 +8,8 @@
 namespace mc {
 
 // Resident 128-thread blocks per SM the register allocator must allow.  Uniform parameters are
-// constant-bank operands, so 3 blocks (<= 168 registers) fit without spills; per-orbit parameters need
-// <= 255 registers (2 blocks).  ptxas -v: 0 spill bytes for all 16 instantiations (profiles/).
+// constant-bank operands, so 3 blocks (<= 168 registers) fit without spills; per-orbit parameters and the
+// quadrupole-monopole term need <= 255 registers (2 blocks; measured as fast, profiles/r01_config_sweep.md).  ptxas -v: 0 spill bytes for all 16 instantiations (profiles/).
 #ifndef MC_MINB_UNIFORM
 #define MC_MINB_UNIFORM 3
 #endif
@@ -18,21 +18,29 @@ namespace mc {
 #endif
 
 template <bool PER_ORBIT, bool QM, int MODE>
-static cudaError_t launch(const McConsts& uc, const IntegrateArgs& A, int grid, cudaStream_t stream, KernelInfo* info) {
-  auto kern = integrate_kernel<PER_ORBIT, QM, MODE, (PER_ORBIT ? MC_MINB_PER_ORBIT : MC_MINB_UNIFORM)>;
+static cudaError_t launch(const McConsts& uc, const IntegrateArgs& A, int num_sms, bool do_launch, cudaStream_t stream,
+                          KernelInfo* info) {
+  auto kern = integrate_kernel<PER_ORBIT, QM, MODE, ((PER_ORBIT || QM) ? MC_MINB_PER_ORBIT : MC_MINB_UNIFORM)>;
   const size_t smem = PER_ORBIT ? sizeof(double) * MC_NCONST * kBlock : 0;
+  cudaFuncAttributes fa;
+  cudaError_t e = cudaFuncGetAttributes(&fa, kern);
+  if (e != cudaSuccess) return e;
+  int bps = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, kBlock, smem);
+  if (e != cudaSuccess) return e;
+  if (bps < 1) return cudaErrorLaunchOutOfResources;
+  const int64_t need = (A.n_units * 32 + kBlock - 1) / kBlock;           // blocks if every unit had its own warp
+  const int64_t cap = (int64_t)num_sms * bps;                              // blocks resident at once
+  const int grid = (int)(need < cap ? need : cap);
   if (info) {
-    cudaFuncAttributes fa;
-    cudaError_t e = cudaFuncGetAttributes(&fa, kern);
-    if (e != cudaSuccess) return e;
     info->regs = fa.numRegs;
     info->local_bytes = (int)fa.localSizeBytes;
     info->block = kBlock;
     info->smem = smem;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&info->blocks_per_sm, kern, kBlock, smem);
-    if (e != cudaSuccess) return e;
+    info->blocks_per_sm = bps;
+    info->grid = grid;
   }
-  if (grid > 0) kern<<<grid, kBlock, smem, stream>>>(uc, A);
+  if (do_launch && grid > 0) kern<<<grid, kBlock, smem, stream>>>(uc, A);
   return cudaGetLastError();
 }
 

@@ -361,3 +361,39 @@ def test_papers_own_scans_match_oracle(mc, which):
     assert calm.sum() >= 0.3 * w.n_orbits
     assert np.abs(gfli[calm] - o.fli[calm]).max() < 1e-2
     assert rel_state_err(gz[:, calm], o.states[:, calm]) < 1e-7
+
+
+def _all_outputs(I, z, n_steps, mode, eps):
+    g = I.integrate(z, 1.0, n_steps, mode, shadow_eps=eps)
+    n = z.shape[1]
+    outs = [g.states, g.invariants, g.status, g.steps_done, I.work(n)] + ([g.fli] if g.fli is not None else [])
+    return [t.cpu().numpy() for t in outs], I.launch_info()
+
+
+@pytest.mark.parametrize("case", ["uniform-shadow", "per-orbit-shadow", "dropped-cells", "mode2-no-shadow"])
+def test_chunked_scheduling_never_changes_a_bit(mc, case):
+    """the kernel's work items are chunks of steps whose state rests in a carry buffer
+    between chunks.  Any chunk length -- a divisor of the run, one that cuts renormalisation intervals, a single
+    step, more chunks than steps -- must reproduce the one-chunk result bit for bit in every output."""
+    mode, eps, kw = 3, 1e-8, {}
+    if case == "uniform-shadow":
+        z = workloads.config0(300).states
+    elif case == "per-orbit-shadow":
+        w = workloads.config3(n_r=9, n_theta=23, qm=True)
+        z, kw = w.states, dict(terms=w.terms, **{k: v for k, v in w.params().items() if k != "terms"})
+    elif case == "dropped-cells":
+        z = workloads.scan_grid(12, 11, r_lo=6.0, r_hi=16.0)[0]
+    else:
+        z, mode, eps = workloads.config0(70).states, 2, 0.0
+    n_steps = 730
+    with mc.Integrator(chunk_steps=n_steps, **kw) as I:
+        ref, info = _all_outputs(I, z, n_steps, mode, eps)
+        assert info["n_chunks"] == 1
+    if case == "dropped-cells":
+        assert (ref[2] != 0).sum() >= 5
+    for chunk in (365, 100, 70, 1, 10_000):
+        with mc.Integrator(chunk_steps=chunk, **kw) as I:
+            got, info = _all_outputs(I, z, n_steps, mode, eps)
+        assert info["n_chunks"] == -(-n_steps // chunk) and info["chunk_steps"] == chunk
+        for a, b in zip(ref, got):
+            assert np.array_equal(a, b, equal_nan=True), (case, chunk)

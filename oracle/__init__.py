@@ -90,6 +90,29 @@ def integrals(z, **kw):
     return evaluate("integrals", z, **kw)
 
 
+RK4, RK5 = 0, 1     # integrator codes (RK5: Butcher's six-stage fifth-order method, R9)
+
+
+def tableau(integrator=RK4):
+    """(c, A, b) of the Butcher tableau the oracle really integrates with."""
+    c, a, b = np.zeros(8), np.zeros(64), np.zeros(8)
+    lib().oracle_tableau.restype = ctypes.c_int
+    s = lib().oracle_tableau(ctypes.c_int(integrator), _p(c), _p(a), _p(b))
+    return c[:s].copy(), a[:s * s].reshape(s, s).copy(), b[:s].copy()
+
+
+def rk_step(z, h, integrator=RK4, beta=1.0, chi1=1.0, chi2=1.0, kq1=1.0, kq2=1.0, terms=TERMS_DEFAULT,
+            precision=LONG_DOUBLE):
+    """One uncorrected step of the base integrator (RK4 or RK5)."""
+    z = _states(z)
+    n = z.shape[1]
+    out = np.empty_like(z)
+    pa = _params(n, beta, chi1, chi2, kq1, kq2)
+    lib().oracle_rk4_step(ctypes.c_int(precision), ctypes.c_int64(n), _p(z), *[_p(a) for a in pa],
+                          ctypes.c_uint32(terms), ctypes.c_double(h), ctypes.c_int(integrator), _p(out))
+    return out
+
+
 def rk4_step(z, h, beta=1.0, chi1=1.0, chi2=1.0, kq1=1.0, kq2=1.0, terms=TERMS_DEFAULT,
              precision=LONG_DOUBLE):
     z = _states(z)
@@ -97,7 +120,7 @@ def rk4_step(z, h, beta=1.0, chi1=1.0, chi2=1.0, kq1=1.0, kq2=1.0, terms=TERMS_D
     out = np.empty_like(z)
     pa = _params(n, beta, chi1, chi2, kq1, kq2)
     lib().oracle_rk4_step(ctypes.c_int(precision), ctypes.c_int64(n), _p(z), *[_p(a) for a in pa],
-                          ctypes.c_uint32(terms), ctypes.c_double(h), _p(out))
+                          ctypes.c_uint32(terms), ctypes.c_double(h), ctypes.c_int(RK4), _p(out))
     return out
 
 
@@ -129,7 +152,7 @@ class Result:
 
 def integrate(z, h, n_steps, mode, shadow_eps=0.0, beta=1.0, chi1=1.0, chi2=1.0, kq1=1.0, kq2=1.0,
               terms=TERMS_DEFAULT, renorm_interval=100, newton_iters=4, newton_tol=1e-10,
-              r_merge=2.0, r_escape=1e4, precision=LONG_DOUBLE, n_threads=0):
+              r_merge=2.0, r_escape=1e4, precision=LONG_DOUBLE, n_threads=0, integrator=RK4):
     """The oracle's statement of mc_integrate (include/mc.h), orbit by orbit."""
     z = _states(z)
     n = z.shape[1]
@@ -142,7 +165,7 @@ def integrate(z, h, n_steps, mode, shadow_eps=0.0, beta=1.0, chi1=1.0, chi2=1.0,
                            ctypes.c_int(newton_iters), ctypes.c_double(newton_tol),
                            ctypes.c_double(r_merge), ctypes.c_double(r_escape), _p(res.states),
                            _p(res.invariants), _p(res.fli), _p(res.status), _p(res.steps_done),
-                           _p(res.gn_steps), ctypes.c_int(n_threads))
+                           _p(res.gn_steps), ctypes.c_int(n_threads), ctypes.c_int(integrator))
     return res
 
 

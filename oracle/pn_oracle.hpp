@@ -216,6 +216,56 @@ template <class T> State<T> rk4_step(const State<T>& z, T h, const Params<T>& P)
   return z + (h / T(6)) * (k1 + T(2) * k2 + T(2) * k3 + k4);
 }
 
+// Explicit Runge-Kutta step with a general Butcher tableau: k_i = f(z + h sum_j a_ij k_j), j < i;
+// z' = z + h sum_i b_i k_i.  Plain loops over the tableau, every k_i stored.
+struct Tableau { int stages; const double* c; const double* a; const double* b; };  // a: row-major [stages][stages]
+
+// The paper integrates with "RK5" without giving a tableau or a step size; reading R9
+// takes Butcher's classical six-stage fifth-order method (J. C. Butcher 1964; c = 0, 1/4, 1/4,
+// 1/2, 3/4, 1; b = 7/90, 0, 32/90, 12/90, 32/90, 7/90).  Its 17 order conditions up to order five are
+// checked on these very arrays in tests/test_oracle_integrator.py.
+inline const Tableau& tableau_rk5() {
+  static const double c[6] = {0.0, 1.0 / 4, 1.0 / 4, 1.0 / 2, 3.0 / 4, 1.0};
+  static const double a[36] = {
+      0, 0, 0, 0, 0, 0,
+      1.0 / 4, 0, 0, 0, 0, 0,
+      1.0 / 8, 1.0 / 8, 0, 0, 0, 0,
+      0, -1.0 / 2, 1.0, 0, 0, 0,
+      3.0 / 16, 0, 0, 9.0 / 16, 0, 0,
+      -3.0 / 7, 2.0 / 7, 12.0 / 7, -12.0 / 7, 8.0 / 7, 0};
+  static const double b[6] = {7.0 / 90, 0, 32.0 / 90, 12.0 / 90, 32.0 / 90, 7.0 / 90};
+  static const Tableau T = {6, c, a, b};
+  return T;
+}
+inline const Tableau& tableau_rk4() {
+  static const double c[4] = {0.0, 0.5, 0.5, 1.0};
+  static const double a[16] = {0, 0, 0, 0, 0.5, 0, 0, 0, 0, 0.5, 0, 0, 0, 0, 1.0, 0};
+  static const double b[4] = {1.0 / 6, 1.0 / 3, 1.0 / 3, 1.0 / 6};
+  static const Tableau T = {4, c, a, b};
+  return T;
+}
+
+template <class T> State<T> rk_step(const State<T>& z, T h, const Params<T>& P, const Tableau& tb) {
+  State<T> k[8];
+  for (int i = 0; i < tb.stages; ++i) {
+    State<T> zi = z;
+    for (int j = 0; j < i; ++j) {
+      const double aij = tb.a[i * tb.stages + j];
+      if (aij != 0.0) zi = zi + (h * T(aij)) * k[j];
+    }
+    k[i] = rhs(zi, P);
+  }
+  State<T> out = z;
+  for (int i = 0; i < tb.stages; ++i)
+    if (tb.b[i] != 0.0) out = out + (h * T(tb.b[i])) * k[i];
+  return out;
+}
+
+// integrator: 0 = classical RK4 (BASELINE), 1 = Butcher's RK5 (the paper's "RK5", reading R9).
+template <class T> State<T> base_step(const State<T>& z, T h, const Params<T>& P, int integrator) {
+  return integrator == 1 ? rk_step(z, h, P, tableau_rk5()) : rk4_step(z, h, P);
+}
+
 // ---- manifold correction ------------------------------------------------------
 template <class T> inline V3<T> unit(V3<T> s) { return (T(1) / o_sqrt(dot(s, s))) * s; }
 
@@ -353,6 +403,7 @@ struct Options {
   int newton_iters;     // Newton iteration cap (mode 3) / fixed count (mode 2), R6
   double newton_tol;    // epsilon of PAPER.md:197: mode 3 termination test, mode 2 convergence flag
   double r_merge, r_escape;  // DESIGN.md R13
+  int integrator;       // 0 classical RK4, 1 Butcher RK5 (R9)
 };
 
 template <class T> struct OrbitResult {
@@ -389,11 +440,11 @@ OrbitResult<T> integrate_orbit(State<T> z, const Params<T>& P, T h, int64_t n_st
   int64_t k = 0, gn_total = 0;
   while (k < n_steps) {
     int gn = 0, gns = 0;
-    State<T> zn = rk4_step(z, h, P);
+    State<T> zn = base_step(z, h, P, O.integrator);
     if (!correct(zn, P, R, O.mode, O.newton_iters, T(O.newton_tol), &gn)) flag = ST_NEWTON_FLAG;
     State<T> zsn = zs;
     if (shadow) {
-      zsn = rk4_step(zs, h, P);
+      zsn = base_step(zs, h, P, O.integrator);
       correct(zsn, P, Rs, O.mode, O.newton_iters, T(O.newton_tol), &gns);
     }
     // status check on the completed step (R13); on failure keep the last good state

@@ -81,10 +81,10 @@ template <class T> void eval_t(int what, int64_t n, const double* states, const 
 }
 
 template <class T>
-void step_t(int64_t n, const double* states, const ParamArrays& A, double h, double* out) {
+void step_t(int64_t n, const double* states, const ParamArrays& A, double h, int integrator, double* out) {
   for (int64_t i = 0; i < n; ++i)
-    store_state(out, n, i, rk4_step(load_state<T>(states, n, i),
-                                    T(h), load_params<T>(A.beta, A.chi1, A.chi2, A.kq1, A.kq2, A.terms, i)));
+    store_state(out, n, i, base_step(load_state<T>(states, n, i),
+                                     T(h), load_params<T>(A.beta, A.chi1, A.chi2, A.kq1, A.kq2, A.terms, i), integrator));
 }
 
 template <class T>
@@ -139,11 +139,19 @@ int oracle_eval(int precision, int what, int64_t n, const double* states, const 
 
 int oracle_rk4_step(int precision, int64_t n, const double* states, const double* beta, const double* chi1,
                     const double* chi2, const double* kq1, const double* kq2, uint32_t terms, double h,
-                    double* out) {
+                    int integrator, double* out) {
   const ParamArrays A = {beta, chi1, chi2, kq1, kq2, terms};
-  if (precision == 0) step_t<long double>(n, states, A, h, out);
-  else step_t<double>(n, states, A, h, out);
+  if (precision == 0) step_t<long double>(n, states, A, h, integrator, out);
+  else step_t<double>(n, states, A, h, integrator, out);
   return 0;
+}
+
+// The Butcher tableau the oracle integrates with (integrator 0 / 1): c[s], a[s*s] row-major, b[s]; returns s.
+int oracle_tableau(int integrator, double* c, double* a, double* b) {
+  const Tableau& T = integrator == 1 ? tableau_rk5() : tableau_rk4();
+  for (int i = 0; i < T.stages; ++i) { c[i] = T.c[i]; b[i] = T.b[i]; }
+  for (int i = 0; i < T.stages * T.stages; ++i) a[i] = T.a[i];
+  return T.stages;
 }
 
 int oracle_correct(int precision, int64_t n, const double* states, const double* beta, const double* chi1,
@@ -161,9 +169,9 @@ int oracle_integrate(int precision, int64_t n, const double* states, const doubl
                      int64_t n_steps, int mode, double shadow_eps, int renorm_interval, int newton_iters,
                      double newton_tol, double r_merge, double r_escape, double* out_states,
                      double* out_invariants, double* out_fli, int32_t* out_status, int64_t* out_step,
-                     int64_t* out_gn_steps, int n_threads) {
+                     int64_t* out_gn_steps, int n_threads, int integrator) {
   const ParamArrays A = {beta, chi1, chi2, kq1, kq2, terms};
-  const Options O = {mode, renorm_interval, newton_iters, newton_tol, r_merge, r_escape};
+  const Options O = {mode, renorm_interval, newton_iters, newton_tol, r_merge, r_escape, integrator};
   if (n_threads <= 0) n_threads = omp_get_max_threads();
   if (precision == 0)
     integrate_t<long double>(n, states, A, h, n_steps, shadow_eps, O, out_states, out_invariants, out_fli,

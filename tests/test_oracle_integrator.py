@@ -252,6 +252,60 @@ def test_newton_termination_rule_of_mode3():
         assert (oracle.integrate(w.states[:, :2], 1.0, 10, mode, **w.subset(np.arange(2)).params()).gn_steps == 0).all()
 
 
+def _order_conditions(c, A, b):
+    """The 17 rooted-tree order conditions of an explicit Runge-Kutta method up to order five
+    (Hairer, Norsett, Wanner, Solving ODEs I, table II.2.x): (left side, right side) pairs."""
+    e = np.ones_like(c)
+    Ac, Ac2, Ac3, AAc = A @ c, A @ c ** 2, A @ c ** 3, A @ (A @ c)
+    return [
+        (b @ e, 1), (b @ c, 1 / 2),                                                    # orders 1, 2
+        (b @ c ** 2, 1 / 3), (b @ Ac, 1 / 6),                                          # order 3
+        (b @ c ** 3, 1 / 4), (b @ (c * Ac), 1 / 8), (b @ Ac2, 1 / 12), (b @ AAc, 1 / 24),   # order 4
+        (b @ c ** 4, 1 / 5), (b @ (c ** 2 * Ac), 1 / 10), (b @ (c * Ac2), 1 / 15), (b @ (c * AAc), 1 / 30),
+        (b @ (Ac * Ac), 1 / 20), (b @ Ac3, 1 / 20), (b @ (A @ (c * Ac)), 1 / 40), (b @ (A @ Ac2), 1 / 60),
+        (b @ (A @ AAc), 1 / 120),                                                      # order 5
+    ]
+
+
+def test_rk5_tableau_satisfies_all_order_conditions_up_to_five():
+    """DESIGN.md R9: the paper's "RK5" has no printed tableau; the oracle uses Butcher's six-stage method.  The
+    arrays the oracle really integrates with must satisfy all 17 order conditions (and sum_j a_ij = c_i); the
+    RK4 tableau satisfies the first 8 and fails the order-5 ones."""
+    c, A, b = oracle.tableau(oracle.RK5)
+    assert len(c) == 6 and np.allclose(A.sum(1), c, atol=1e-16) and np.all(np.triu(A) == 0)
+    for lhs, rhs in _order_conditions(c, A, b):
+        assert abs(lhs - rhs) < 2e-16
+    c4, A4, b4 = oracle.tableau(oracle.RK4)
+    cond4 = _order_conditions(c4, A4, b4)
+    assert all(abs(l - r) < 2e-16 for l, r in cond4[:8]) and any(abs(l - r) > 1e-3 for l, r in cond4[8:])
+
+
+def test_rk5_reproduces_kepler_orbit_with_fifth_order_convergence():
+    a, e = 12.0, 0.3
+    T = 2 * np.pi * a ** 1.5
+    errs = []
+    for n in (200, 400, 800):
+        o = oracle.integrate(kepler_z0(a, e), T / n, n, mode=0, terms=0, integrator=oracle.RK5, r_merge=0.0)
+        errs.append(np.abs(o.states[0:6, 0] - kepler_state(a, e, T)).max())
+    assert errs[0] < 1e-3 and 27 < errs[0] / errs[1] < 37 and 27 < errs[1] / errs[2] < 37   # 2^5 = 32
+    one4 = oracle.rk_step(kepler_z0(a, e), 1.0, oracle.RK4, terms=0)
+    one4b = oracle.rk4_step(kepler_z0(a, e), 1.0, terms=0)
+    assert np.array_equal(one4, one4b)
+
+
+def test_rk5_with_correction_keeps_the_integrals_and_beats_rk4_accuracy():
+    w = workloads.paper_orbit(2)
+    ref = oracle.integrate(w.states, 0.125, 8 * 2000, 0, integrator=oracle.RK5, **w.params())     # fine-step reference
+    out = {}
+    for integ in (oracle.RK4, oracle.RK5):
+        o = oracle.integrate(w.states, 1.0, 2000, 3, integrator=integ, **w.params())
+        I1 = oracle.integrals(o.states, **w.params())
+        assert abs(I1[0, 0] / o.invariants[0, 0] - 1) < 1e-14
+        assert np.abs(I1[1:4, 0] - o.invariants[1:4, 0]).max() < 1e-14
+        out[integ] = np.abs(o.states[0:3, 0] - ref.states[0:3, 0]).max()
+    assert out[oracle.RK5] < 0.2 * out[oracle.RK4]
+
+
 def test_flop_counter_reports_the_oracles_own_formulation():
     c = oracle.count_flops(workloads.paper_orbit(2).states[:, 0], terms=15, mode=3, newton_iters=2)
     assert c["rk4_step"] == 4 * c["rhs"] + 159            # 3 stage inputs (3*25) + final combination (84)

@@ -32,10 +32,11 @@ UNIT = "orbit-steps/s"
 # The number of Gauss-Newton steps is data dependent (epsilon-terminated, R6): the kernel counts
 # them (mc_get_work) and the flop total of a launch is 2270 x accepted orbit-steps + 390 x counted steps.
 # The oracle's unfactored formulation needs about twice as much (oracle.count_flops): conservative.
-# DRAM traffic of one launch of the hot kernel on the default workload, from the ncu --set full capture
-# (profiles/r01b_ncu_integrate_kernel_mode3.md: dram__bytes_read.sum + dram__bytes_write.sum); the outputs
-# (31 MB) stay in the 126 MB L2 until after the kernel.  Algorithmic: 340 B per orbit.
-NCU_DRAM_BYTES_PER_LAUNCH_314 = 9.507e6
+# DRAM traffic of one launch of the hot kernel on the default grid, from the ncu --set full capture
+# (profiles/r01c_ncu_integrate_kernel_mode3.md: dram__bytes_read.sum + dram__bytes_write.sum = 9.64 + 5.20 MB
+# for a 4000-step launch; ncu replays make a 1e5-step capture impractical).  Outputs (31 MB) and the carry
+# buffer (31 MB) live in the 126 MB L2.  Algorithmic: 340 B per orbit.
+NCU_DRAM_BYTES_PER_LAUNCH_314 = 14.84e6
 FLOP_PER_ORBIT_STEP_BASE = 2270.0
 FLOP_PER_GN_STEP = 390.0
 FP64_LANES_PER_SM = 64
@@ -303,7 +304,7 @@ def run_mc(args):
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": nominal_tf, "unit": "TFLOP/s",
                 "frac": achieved_tf / nominal_tf,
                 "traffic": NCU_DRAM_BYTES_PER_LAUNCH_314 if (w.name.startswith("config2") and args.grid == 314 and world == 1) else None,
-                "traffic_unit": "bytes per launch (ncu capture, profiles/r01b_ncu_integrate_kernel_mode3.md)",
+                "traffic_unit": "bytes per launch (ncu capture of a 4000-step launch, profiles/r01c_ncu_integrate_kernel_mode3.md)",
                 "algorithmic_bytes_per_launch": 340.0 * n,
                 "peak_source": f"derived: {info['num_sms']} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x {sm_max:.0f} MHz "
                                "(MEASURED_PEAKS.json has no FP64 entry)",

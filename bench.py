@@ -39,6 +39,8 @@ UNIT = "orbit-steps/s"
 NCU_DRAM_BYTES_PER_LAUNCH_314 = 14.84e6
 FLOP_PER_ORBIT_STEP_BASE = 2270.0
 FLOP_PER_GN_STEP = 390.0
+# RK5 (Butcher, 6 stages): 2 x [6 x 229 + 408 (stage sums: 204 FMA) + 34 + 12 + 5] = 3666
+FLOP_PER_ORBIT_STEP_BASE_RK5 = 3666.0
 FP64_LANES_PER_SM = 64
 
 
@@ -54,6 +56,8 @@ def parse_args():
                     help="config2 (default, the bench line) | config0 | config1 | config1:mode0 | config3 | config3:qmoff | "
                          "config4:<log2 n> | paper-theta2 | paper-theta2:0 | paper-plane  -- the other BASELINE configs and the "
                          "paper's own scans (PAPER.md:227), for profiles/ tables only")
+    ap.add_argument("--integrator", default="rk4", choices=["rk4", "rk5"],
+                    help="rk4 (BASELINE, default) | rk5 (Butcher six-stage, the paper's 'RK5'; profiles/ tables only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -138,12 +142,13 @@ def rank_shard(w, args, rank, world):
 
 
 def describe(w, args):
+    integ = "RK5 (Butcher six-stage)" if args.integrator == "rk5" else "RK4"
     if w.name.startswith("config2"):
         return (f"config2: {args.grid}x{args.grid} orbit scan per GPU (r0 in [10,60] x theta in [0,pi]), equal mass, chi=1, "
-                f"N+1PN+2PN+SO+SS, RK4 h=1, {w.n_steps} steps, shadow 1e-8 renormalised every 100 steps + FLI, "
+                f"N+1PN+2PN+SO+SS, {integ} h=1, {w.n_steps} steps, shadow 1e-8 renormalised every 100 steps + FLI, "
                 "six-integral correction (mode 3, Gauss-Newton terminated at eps=1e-10, cap 4)")
     return (f"{args.workload} ({w.name}): {w.n_orbits} orbits per GPU, terms mask {w.terms}, "
-            f"{'uniform' if w.uniform else 'per-orbit'} parameters, RK4 h={w.h}, {w.n_steps} steps, shadow {w.shadow_eps}, "
+            f"{'uniform' if w.uniform else 'per-orbit'} parameters, {integ} h={w.h}, {w.n_steps} steps, shadow {w.shadow_eps}, "
             f"correction mode {w.correction_mode}")
 
 
@@ -234,7 +239,8 @@ def run_mc(args):
         par = dict(beta=float(w.beta[0]), chi1=float(w.chi1[0]), chi2=float(w.chi2[0]), kq1=float(w.kq1[0]), kq2=float(w.kq2[0]))
     else:
         par = {k: v for k, v in w.params().items() if k != "terms"}
-    I = binding.Integrator(terms=w.terms, device=local, **par)
+    rk5 = args.integrator == "rk5"
+    I = binding.Integrator(terms=w.terms, device=local, integrator=int(rk5), **par)
     out = torch.empty_like(z_dev)
     stream = torch.cuda.current_stream(dev)
     launches = 0
@@ -299,7 +305,8 @@ def run_mc(args):
     sm_max = float(mp.get("sm_max_mhz", clocks.get("sm_max_mhz") or 1965.0))
     nominal_tf = info["num_sms"] * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     per_launch_s = (dev_ms / args.steps) * 1e-3
-    flop_per_launch = FLOP_PER_ORBIT_STEP_BASE * steps_done + FLOP_PER_GN_STEP * gn_steps
+    base = FLOP_PER_ORBIT_STEP_BASE_RK5 if rk5 else FLOP_PER_ORBIT_STEP_BASE
+    flop_per_launch = base * steps_done + FLOP_PER_GN_STEP * gn_steps
     achieved_tf = flop_per_launch / per_launch_s / 1e12
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": nominal_tf, "unit": "TFLOP/s",
                 "frac": achieved_tf / nominal_tf,

@@ -57,6 +57,13 @@ enum mc_status {
   MC_ST_NEWTON_FLAG = 256 /* OR-ed in: mode 2 skipped its (r,p) scaling on >= 1 step (R7) */
 };
 
+/* Base integrator (R9).  BASELINE.json fixes classical RK4; the paper itself says "RK5"
+ * without a tableau, read as Butcher's six-stage fifth-order method. */
+enum mc_integrator {
+  MC_INTEG_RK4 = 0,   /* c = 0, 1/2, 1/2, 1; b = 1/6, 1/3, 1/3, 1/6                                        */
+  MC_INTEG_RK5 = 1    /* c = 0, 1/4, 1/4, 1/2, 3/4, 1; b = 7/90, 0, 32/90, 12/90, 32/90, 7/90                */
+};
+
 typedef struct mc_params {
   uint32_t struct_size;   /* = sizeof(mc_params); checked by mc_create                                   */
   uint32_t terms;         /* OR of mc_terms                                                              */
@@ -82,19 +89,20 @@ typedef struct mc_params {
   int32_t chunk_steps;     /* scheduling only, never changes a result bit: 0 = automatic; > 0 = the kernel's
                               work items are chunks of this many steps (state parked in device scratch owned
                               by the handle between chunks)                          */
+  int32_t integrator;      /* mc_integrator; default MC_INTEG_RK4                                          */
 } mc_params;
 
 /* Fill *p with defaults: terms = 1PN|2PN|SO|S1S2, device 0, uniform beta = chi = kq = 1,
  * renorm_interval 100, newton_iters 4, newton_tol 1e-10, r_merge 2, r_escape 1e4, stream NULL,
- * chunk_steps 0. */
+ * chunk_steps 0, integrator RK4. */
 int mc_params_default(mc_params* p);
 
 /* Validate params, select the device, allocate the handle.  *out_handle is set only on success. */
 int mc_create(const mc_params* params, mc_handle** out_handle);
 
-/* Integrate n_orbits independent orbits for n_steps classical RK4 steps of size step_h (may be
- * negative), applying correction_mode after every step (the per-orbit algorithm
- * is spelled out in DESIGN.md section 2).  Reference integrals E0, J0 are taken from the input states
+/* Integrate n_orbits independent orbits for n_steps steps of size step_h (may be negative) of the base
+ * integrator (classical RK4 unless params.integrator says RK5), applying correction_mode after every
+ * step (the per-orbit algorithm is spelled out in DESIGN.md section 2).  Reference integrals E0, J0 are taken from the input states
  * (PAPER.md:136); with correction_mode >= 1 the input spins are normalised first.
  *
  * shadow_eps != 0 adds, per orbit, a shadow trajectory started at rx + shadow_eps, integrated and
@@ -138,7 +146,7 @@ int mc_get_work(mc_handle* h, int64_t* out_gn_steps);
  *   what = 0: out[1][n]  = H                     (eq 1)
  *   what = 1: out[12][n] = dz/dt                 (eqs 6-9: dH/dp, -dH/dr, Omega_i x S_i_hat)
  *   what = 2: out[6][n]  = E, Jx, Jy, Jz, |S1hat|, |S2hat|
- *   what = 3: out[12][n] = one RK4 step of size step_h, no correction
+ *   what = 3: out[12][n] = one step of the base integrator (params.integrator) of size step_h, no correction
  *   what = 4: out[12][n] = correction operator of mode `mode` applied to states, with references
  *             refs = DEVICE double[4][n] (E0, J0x, J0y, J0z)
  * Asynchronous on the handle's stream. */
@@ -153,7 +161,7 @@ typedef struct mc_launch_info {
   int32_t blocks_per_sm;        /* occupancy API result for that block size       */
   int32_t num_sms;
   int32_t smem_bytes;           /* dynamic shared memory per block                */
-  int32_t variant;              /* bit0 per-orbit params, bit1 QM, bits 4-5 mode  */
+  int32_t variant;              /* bit0 per-orbit params, bit1 QM, bits 4-5 mode, bit 8 RK5 */
   int64_t trajectories;         /* threads doing work = n_orbits * (1 + shadow)   */
   int32_t chunk_steps;          /* steps per work item                             */
   int32_t n_chunks;             /* work items per 32-trajectory unit              */

@@ -14,6 +14,7 @@ from . import build as _build
 MC_TERM_1PN, MC_TERM_2PN, MC_TERM_SO, MC_TERM_S1S2, MC_TERM_QM = 1, 2, 4, 8, 16
 TERMS_DEFAULT = MC_TERM_1PN | MC_TERM_2PN | MC_TERM_SO | MC_TERM_S1S2
 MC_OK, MC_EINVAL, MC_ECUDA, MC_EARCH, MC_ENOMEM = 0, -1, -2, -3, -4
+MC_INTEG_RK4, MC_INTEG_RK5 = 0, 1
 
 # every symbol include/mc.h declares (tests/test_abi.py checks the header against this list)
 EXPORTS = ["mc_params_default", "mc_create", "mc_integrate", "mc_integrate_host", "mc_get_status", "mc_get_work", "mc_eval",
@@ -37,7 +38,7 @@ class mc_params(ctypes.Structure):
                 ("d_beta", ctypes.c_void_p), ("d_chi1", ctypes.c_void_p), ("d_chi2", ctypes.c_void_p),
                 ("d_kq1", ctypes.c_void_p), ("d_kq2", ctypes.c_void_p), ("renorm_interval", ctypes.c_int32),
                 ("newton_iters", ctypes.c_int32), ("newton_tol", ctypes.c_double), ("r_merge", ctypes.c_double),
-                ("r_escape", ctypes.c_double), ("cuda_stream", ctypes.c_void_p), ("chunk_steps", ctypes.c_int32)]
+                ("r_escape", ctypes.c_double), ("cuda_stream", ctypes.c_void_p), ("chunk_steps", ctypes.c_int32), ("integrator", ctypes.c_int32)]
 
 
 class mc_launch_info(ctypes.Structure):
@@ -123,7 +124,7 @@ class Integrator:
 
     def __init__(self, terms=TERMS_DEFAULT, beta=1.0, chi1=1.0, chi2=1.0, kq1=1.0, kq2=1.0, device=0,
                  renorm_interval=100, newton_iters=4, newton_tol=1e-10, r_merge=2.0, r_escape=1e4, stream=None,
-                 chunk_steps=0):
+                 chunk_steps=0, integrator=0):
         import torch
         self._torch = torch
         self._lib = load_library()
@@ -132,6 +133,7 @@ class Integrator:
         p.renorm_interval, p.newton_iters, p.newton_tol = int(renorm_interval), int(newton_iters), float(newton_tol)
         p.r_merge, p.r_escape = float(r_merge), float(r_escape)
         p.chunk_steps = int(chunk_steps)
+        p.integrator = int(integrator)
         self.device = torch.device("cuda", device)
         vals = dict(beta=beta, chi1=chi1, chi2=chi2, kq1=kq1, kq2=kq2)
         per_orbit = any(hasattr(v, "__len__") for v in vals.values())

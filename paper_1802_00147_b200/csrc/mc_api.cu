@@ -100,7 +100,8 @@ eval_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ mc::Int
     mc::six_integrals<QM>(c, z, f);
     rows = 6;
   } else if (what == 3) {
-    mc::rk4_step<QM>(c, z, A.h, f);
+    if (A.integrator == 1) mc::rk5_step<QM>(c, z, A.h, f);
+    else mc::rk4_step<QM>(c, z, A.h, f);
   } else {
     mc::Refs R;
     R.E0 = refs[o];
@@ -147,6 +148,7 @@ void fill_args(const mc_handle* h, mc::IntegrateArgs& A) {
   A.renorm_interval = h->P.renorm_interval;
   A.newton_iters = h->P.newton_iters;
   A.newton_tol = h->P.newton_tol;
+  A.integrator = h->P.integrator;
   A.r_merge2 = h->P.r_merge * h->P.r_merge;
   A.r_escape2 = h->P.r_escape * h->P.r_escape;
 }
@@ -170,6 +172,7 @@ int mc_params_default(mc_params* p) {
   p->r_escape = 1e4;
   p->cuda_stream = nullptr;
   p->chunk_steps = 0;
+  p->integrator = MC_INTEG_RK4;
   return MC_OK;
 }
 
@@ -179,6 +182,7 @@ int mc_create(const mc_params* params, mc_handle** out_handle) {
   if (params->terms & ~31u) return MC_EINVAL;
   if (params->renorm_interval <= 0 || params->newton_iters < 1 || params->newton_iters > 16) return MC_EINVAL;
   if (params->chunk_steps < 0) return MC_EINVAL;
+  if (params->integrator != MC_INTEG_RK4 && params->integrator != MC_INTEG_RK5) return MC_EINVAL;
   if (!(params->newton_tol >= 0.0) || !(params->r_merge >= 0.0) || !(params->r_escape > params->r_merge)) return MC_EINVAL;
   if (params->per_orbit) {
     if (!params->d_beta || !params->d_chi1 || !params->d_chi2 || !params->d_kq1 || !params->d_kq2) return MC_EINVAL;
@@ -233,10 +237,10 @@ int mc_integrate(mc_handle* h, const double* states, int64_t n_orbits, double st
   const bool qm = (h->P.terms & MC_TERM_QM) != 0;
   mc::LaunchFn fn = nullptr;
   switch (correction_mode) {
-    case 0: fn = mc::launcher_mode0(h->P.per_orbit != 0, qm); break;
-    case 1: fn = mc::launcher_mode1(h->P.per_orbit != 0, qm); break;
-    case 2: fn = mc::launcher_mode2(h->P.per_orbit != 0, qm); break;
-    default: fn = mc::launcher_mode3(h->P.per_orbit != 0, qm); break;
+    case 0: fn = mc::launcher_mode0(h->P.per_orbit != 0, qm, h->P.integrator); break;
+    case 1: fn = mc::launcher_mode1(h->P.per_orbit != 0, qm, h->P.integrator); break;
+    case 2: fn = mc::launcher_mode2(h->P.per_orbit != 0, qm, h->P.integrator); break;
+    default: fn = mc::launcher_mode3(h->P.per_orbit != 0, qm, h->P.integrator); break;
   }
   const int64_t traj = n_orbits * (shadow ? 2 : 1);
   A.n_units = (traj + 31) / 32;
@@ -284,7 +288,7 @@ int mc_integrate(mc_handle* h, const double* states, int64_t n_orbits, double st
   h->info.blocks_per_sm = ki.blocks_per_sm;
   h->info.num_sms = h->num_sms;
   h->info.smem_bytes = (int32_t)ki.smem;
-  h->info.variant = (h->P.per_orbit ? 1 : 0) | (qm ? 2 : 0) | (correction_mode << 4);
+  h->info.variant = (h->P.per_orbit ? 1 : 0) | (qm ? 2 : 0) | (correction_mode << 4) | (h->P.integrator << 8);
   h->info.trajectories = traj;
   return MC_OK;
 }

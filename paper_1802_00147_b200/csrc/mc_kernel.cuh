@@ -36,6 +36,7 @@ struct IntegrateArgs {
   uint32_t terms;
   int32_t renorm_interval;
   int32_t newton_iters;
+  int32_t integrator;         // 0 RK4, 1 RK5 (mc_eval only; integrate_kernel is instantiated per integrator)
   // scheduling
   unsigned long long* queue;  // [0] = next item
   int32_t* done;              // [n_units] chunks completed per unit
@@ -71,7 +72,7 @@ __device__ __forceinline__ void six_integrals(const C& c, const double* z, doubl
 #define MC_KERNEL_BOUNDS(MINB) __launch_bounds__(kBlock, MINB)
 #endif
 
-template <bool PER_ORBIT, bool QM, int MODE, int MINB>
+template <bool PER_ORBIT, bool QM, int MODE, int INTEG, int MINB>
 __global__ void MC_KERNEL_BOUNDS(MINB)
 integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ IntegrateArgs A) {
   extern __shared__ double smem[];   // PER_ORBIT: [MC_NCONST][kBlock]
@@ -160,7 +161,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
     for (int k = chunk * A.chunk_len; k < k_end; ++k) {
       if (__all_sync(0xffffffffu, frozen)) break;
       double z[12];
-      rk4_step<QM>(c, y, A.h, z);
+      base_step<INTEG, QM>(c, y, A.h, z);
       int gn;
       const bool ok = correct<MODE, QM>(c, z, R, A.newton_iters, A.newton_tol, gn);
       if (MODE == 2 && !ok && !role_shadow && !frozen) flag = ST_NEWTON_FLAG;

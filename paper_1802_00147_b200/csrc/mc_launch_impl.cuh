@@ -8,8 +8,8 @@
 namespace mc {
 
 // Resident 128-thread blocks per SM the register allocator must allow.  Uniform parameters are
-// constant-bank operands, so 3 blocks (<= 168 registers) fit without spills; per-orbit parameters and the
-// quadrupole-monopole term need <= 255 registers (2 blocks; measured as fast, profiles/r01_config_sweep.md).  ptxas -v: 0 spill bytes for all 16 instantiations (profiles/).
+// constant-bank operands, so 3 blocks (<= 168 registers) fit without spills; per-orbit parameters, the
+// quadrupole-monopole term and the six-stage RK5 need <= 255 registers (2 blocks; measured as fast, profiles/r01_config_sweep.md).  ptxas -v: 0 spill bytes for all 16 instantiations (profiles/).
 #ifndef MC_MINB_UNIFORM
 #define MC_MINB_UNIFORM 3
 #endif
@@ -17,10 +17,10 @@ namespace mc {
 #define MC_MINB_PER_ORBIT 2
 #endif
 
-template <bool PER_ORBIT, bool QM, int MODE>
+template <bool PER_ORBIT, bool QM, int MODE, int INTEG>
 static cudaError_t launch(const McConsts& uc, const IntegrateArgs& A, int num_sms, bool do_launch, cudaStream_t stream,
                           KernelInfo* info) {
-  auto kern = integrate_kernel<PER_ORBIT, QM, MODE, ((PER_ORBIT || QM) ? MC_MINB_PER_ORBIT : MC_MINB_UNIFORM)>;
+  auto kern = integrate_kernel<PER_ORBIT, QM, MODE, INTEG, ((PER_ORBIT || QM || INTEG == 1) ? MC_MINB_PER_ORBIT : MC_MINB_UNIFORM)>;
   const size_t smem = PER_ORBIT ? sizeof(double) * MC_NCONST * kBlock : 0;
   cudaFuncAttributes fa;
   cudaError_t e = cudaFuncGetAttributes(&fa, kern);
@@ -44,10 +44,15 @@ static cudaError_t launch(const McConsts& uc, const IntegrateArgs& A, int num_sm
   return cudaGetLastError();
 }
 
+template <int MODE, int INTEG>
+static LaunchFn pick2(bool per_orbit, bool qm) {
+  if (per_orbit) return qm ? launch<true, true, MODE, INTEG> : launch<true, false, MODE, INTEG>;
+  return qm ? launch<false, true, MODE, INTEG> : launch<false, false, MODE, INTEG>;
+}
+
 template <int MODE>
-static LaunchFn pick(bool per_orbit, bool qm) {
-  if (per_orbit) return qm ? launch<true, true, MODE> : launch<true, false, MODE>;
-  return qm ? launch<false, true, MODE> : launch<false, false, MODE>;
+static LaunchFn pick(bool per_orbit, bool qm, int integrator) {
+  return integrator == 1 ? pick2<MODE, 1>(per_orbit, qm) : pick2<MODE, 0>(per_orbit, qm);
 }
 
 }  // namespace mc

@@ -194,6 +194,61 @@ __device__ __forceinline__ void rk4_step(const C& c, const double* y, double h, 
   for (int i = 0; i < 12; ++i) out[i] = fma(h6, k[i], out[i]);
 }
 
+// Butcher's six-stage fifth-order method (the paper's "RK5", R9):
+//   c = 0, 1/4, 1/4, 1/2, 3/4, 1;  b = 7/90, 0, 32/90, 12/90, 32/90, 7/90
+//   a2 = (1/4); a3 = (1/8, 1/8); a4 = (0, -1/2, 1); a5 = (3/16, 0, 0, 9/16); a6 = (-3/7, 2/7, 12/7, -12/7, 8/7)
+// Bookkeeping: the linear combinations needed later (stage-4 input, stage-6 input, final sum) are accumulated as
+// the stages arrive, so at most five 12-vectors are live besides the derivative being computed.
+template <bool QM, class C>
+__device__ __forceinline__ void rk5_step(const C& c, const double* y, double h, double* out) {
+  double k[12], k1[12], yt[12], A4[12], S6[12];
+  pn_rhs<QM>(c, y, k1);
+  const double h4 = 0.25 * h, h8 = 0.125 * h;
+#pragma unroll
+  for (int i = 0; i < 12; ++i) yt[i] = fma(h4, k1[i], y[i]);
+  pn_rhs<QM>(c, yt, k);                                                    // k2
+  const double hm2 = -0.5 * h, h37 = h * (-3.0 / 7.0), h27 = h * (2.0 / 7.0);
+#pragma unroll
+  for (int i = 0; i < 12; ++i) {
+    yt[i] = fma(h8, k[i], fma(h8, k1[i], y[i]));
+    A4[i] = fma(hm2, k[i], y[i]);
+    S6[i] = fma(h27, k[i], fma(h37, k1[i], y[i]));
+  }
+  pn_rhs<QM>(c, yt, k);                                                    // k3
+  const double h127 = h * (12.0 / 7.0), h790 = h * (7.0 / 90.0), h3290 = h * (32.0 / 90.0);
+#pragma unroll
+  for (int i = 0; i < 12; ++i) {
+    yt[i] = fma(h, k[i], A4[i]);
+    S6[i] = fma(h127, k[i], S6[i]);
+    out[i] = fma(h3290, k[i], fma(h790, k1[i], y[i]));
+  }
+  pn_rhs<QM>(c, yt, k);                                                    // k4
+  const double h316 = h * (3.0 / 16.0), h916 = h * (9.0 / 16.0), h1290 = h * (12.0 / 90.0);
+#pragma unroll
+  for (int i = 0; i < 12; ++i) {
+    yt[i] = fma(h916, k[i], fma(h316, k1[i], y[i]));
+    S6[i] = fma(-h127, k[i], S6[i]);
+    out[i] = fma(h1290, k[i], out[i]);
+  }
+  pn_rhs<QM>(c, yt, k);                                                    // k5
+  const double h87 = h * (8.0 / 7.0);
+#pragma unroll
+  for (int i = 0; i < 12; ++i) {
+    yt[i] = fma(h87, k[i], S6[i]);
+    out[i] = fma(h3290, k[i], out[i]);
+  }
+  pn_rhs<QM>(c, yt, k);                                                    // k6
+#pragma unroll
+  for (int i = 0; i < 12; ++i) out[i] = fma(h790, k[i], out[i]);
+}
+
+// INTEG: 0 classical RK4, 1 Butcher RK5
+template <int INTEG, bool QM, class C>
+__device__ __forceinline__ void base_step(const C& c, const double* y, double h, double* out) {
+  if (INTEG == 1) rk5_step<QM>(c, y, h, out);
+  else rk4_step<QM>(c, y, h, out);
+}
+
 // eq (10): sigma <- sigma / |sigma|
 __device__ __forceinline__ void normalise3(double* s) {
   const double w = rsqrt_pos(dot3(s, s));

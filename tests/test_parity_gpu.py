@@ -397,3 +397,37 @@ def test_chunked_scheduling_never_changes_a_bit(mc, case):
         assert info["n_chunks"] == -(-n_steps // chunk) and info["chunk_steps"] == chunk
         for a, b in zip(ref, got):
             assert np.array_equal(a, b, equal_nan=True), (case, chunk)
+
+
+def test_rk5_base_integrator_matches_oracle(mc):
+    """SURVEY 8(f) row 2 / DESIGN.md R9: Butcher's six-stage RK5 as the base integrator (the paper's "RK5").
+    One uncorrected step on random states, then config 0 (1e3 steps, mode 3) and a shadowed per-orbit case."""
+    z = random_states(300, seed=5)
+    par = PARAM_SETS[1]
+    for terms in (15, 31):
+        with mc.Integrator(terms=terms, integrator=mc.MC_INTEG_RK5, **par) as I:
+            got = I.eval("rk4_step", z, h=1.0).cpu().numpy()                  # what = 3: one base-integrator step
+        want = oracle.rk_step(z, 1.0, oracle.RK5, terms=terms, **par)
+        assert rel_state_err_blocks(got, want) < 2e-13
+        assert rel_state_err_blocks(got, oracle.rk4_step(z, 1.0, terms=terms, **par)) > 1e-9      # really another method
+    w = workloads.config0()
+    with mc.Integrator(integrator=mc.MC_INTEG_RK5) as I:
+        g = I.integrate(w.states, 1.0, 1000, 3)
+        info = I.launch_info()
+    o = oracle.integrate(w.states, 1.0, 1000, 3, integrator=oracle.RK5, **w.params())
+    assert info["local_bytes"] == 0 and (info["variant"] >> 8) & 1 == 1
+    assert rel_state_err(g.states.cpu().numpy(), o.states) <= STATE_RTOL
+    assert drift(g.states.cpu().numpy(), o.invariants[0:6], **w.params()) <= DRIFT_TOL
+    assert np.array_equal(g.steps_done.cpu().numpy(), o.steps_done)
+    w = workloads.config1().subset(np.arange(150))
+    kw = {k: v for k, v in w.params().items() if k != "terms"}
+    with mc.Integrator(terms=w.terms, integrator=mc.MC_INTEG_RK5, **kw) as I:
+        g = I.integrate(w.states, 1.0, 1500, 3, shadow_eps=1e-8)
+    with mc.Integrator(terms=w.terms, integrator=mc.MC_INTEG_RK5, chunk_steps=170, **kw) as I:
+        gc = I.integrate(w.states, 1.0, 1500, 3, shadow_eps=1e-8)
+    o = oracle.integrate(w.states, 1.0, 1500, 3, shadow_eps=1e-8, integrator=oracle.RK5, **w.params())
+    assert rel_state_err(g.states.cpu().numpy(), o.states) <= 4 * STATE_RTOL
+    assert np.abs(g.fli.cpu().numpy() - o.fli).max() < 1e-3
+    assert np.array_equal(g.status.cpu().numpy(), o.status)
+    assert np.array_equal(g.states.cpu().numpy(), gc.states.cpu().numpy())       # chunking: bit-identical
+    assert np.array_equal(g.fli.cpu().numpy(), gc.fli.cpu().numpy())

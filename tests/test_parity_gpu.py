@@ -431,3 +431,48 @@ def test_rk5_base_integrator_matches_oracle(mc):
     assert np.array_equal(g.status.cpu().numpy(), o.status)
     assert np.array_equal(g.states.cpu().numpy(), gc.states.cpu().numpy())       # chunking: bit-identical
     assert np.array_equal(g.fli.cpu().numpy(), gc.fli.cpu().numpy())
+
+
+def test_step_size_and_tolerance_studies(mc):
+    """convergence in h for both base integrators and the Newton-tolerance study of
+    PAPER.md:195-197 (epsilon = 1e-6, 1e-8, 1e-10) for the mode-3 correction.  Prints the tables recorded in
+    profiles/r01_rk5_and_studies.md (run with -s)."""
+    w = workloads.paper_orbit(1)                                     # PAPER.md:193 orbit 1 (regular), beta = 1/3, chi = 0.75
+    par = dict(beta=float(w.beta[0]), chi1=float(w.chi1[0]), chi2=float(w.chi2[0]))
+    t_end = 2048
+    ref = oracle.integrate(w.states, 0.0625, t_end * 16, 0, integrator=oracle.RK5, **w.params()).states[:, 0]
+    print("\\nh-study, paper orbit 1, uncorrected, t = %d: max |r - r_ref|" % t_end)
+    errs = {}
+    for integ, name in ((mc.MC_INTEG_RK4, "RK4"), (mc.MC_INTEG_RK5, "RK5")):
+        with mc.Integrator(integrator=integ, **par) as I:
+            for h in (4.0, 2.0, 1.0, 0.5):
+                g = I.integrate(w.states, h, int(t_end / h), 0).states.cpu().numpy()[:, 0]
+                errs[name, h] = np.abs(g[0:3] - ref[0:3]).max()
+        print("  %s: " % name + "  ".join("h=%g: %.3e" % (h, errs[name, h]) for h in (4.0, 2.0, 1.0, 0.5)))
+    assert 12 < errs["RK4", 2.0] / errs["RK4", 1.0] < 20 and 12 < errs["RK4", 4.0] / errs["RK4", 2.0] < 20     # 2^4
+    assert 25 < errs["RK5", 4.0] / errs["RK5", 2.0] < 40 and 25 < errs["RK5", 2.0] / errs["RK5", 1.0] < 40     # 2^5
+    assert errs["RK5", 1.0] < 0.1 * errs["RK4", 1.0]
+
+    w0 = workloads.config0()
+    print("epsilon-study, config 0 (64 orbits), RK4 h = 1, 1e4 steps, mode 3, cap 4: max relative drift of E, J; "
+          "Gauss-Newton steps per step")
+    res = {}
+    for eps in (1e-4, 1e-6, 1e-8, 1e-10, 0.0):
+        with mc.Integrator(newton_tol=eps) as I:
+            g = I.integrate(w0.states, 1.0, 10_000, 3)
+            gn = I.work(64).cpu().numpy().mean() / 10_000
+        inv0 = g.invariants.cpu().numpy()[0:6]
+        I1 = oracle.integrals(g.states.cpu().numpy(), **w0.params())
+        dE = (np.abs(I1[0] - inv0[0]) / np.abs(inv0[0])).max()
+        dJ = (np.linalg.norm(I1[1:4] - inv0[1:4], axis=0) / np.linalg.norm(inv0[1:4], axis=0)).max()
+        res[eps] = (dE, dJ, gn)
+        print("  eps=%-6g dE=%.2e dJ=%.2e steps=%.3f" % (eps, dE, dJ, gn))
+    with mc.Integrator() as I:
+        g0 = I.integrate(w0.states, 1.0, 10_000, 0)
+    E0 = oracle.integrals(w0.states, **w0.params())[0]
+    dE0 = (np.abs(oracle.integrals(g0.states.cpu().numpy(), **w0.params())[0] - E0) / np.abs(E0)).max()
+    print("  uncorrected RK4: dE=%.2e" % dE0)
+    assert dE0 > 1e-9                                                  # the correction has work to do
+    assert max(res[1e-10][0:2]) <= DRIFT_TOL and max(res[1e-8][0:2]) <= DRIFT_TOL
+    assert res[1e-4][2] <= res[1e-8][2] <= res[0.0][2] and res[0.0][2] > 2.5    # eps = 0: runs to the cap
+    assert res[1e-4][2] < 1.05                                          # loose tolerance: one step per step

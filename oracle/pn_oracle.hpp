@@ -421,8 +421,11 @@ template <class T> inline void six_integrals(const State<T>& z, const Params<T>&
   out[4] = o_sqrt(dot(z.s1, z.s1)); out[5] = o_sqrt(dot(z.s2, z.s2));
 }
 
-template <class T>
-OrbitResult<T> integrate_orbit(State<T> z, const Params<T>& P, T h, int64_t n_steps, T shadow_eps, const Options& O) {
+// sampler(s, z): optional callback, called after every sample_interval-th step index (k = interval, 2 interval,
+// ...) with the orbit's current state -- the frozen state once the orbit has been dropped.
+template <class T, class Sampler>
+OrbitResult<T> integrate_orbit(State<T> z, const Params<T>& P, T h, int64_t n_steps, T shadow_eps, const Options& O,
+                               int64_t sample_interval, Sampler sampler) {
   OrbitResult<T> out;
   const bool shadow = !(shadow_eps == T(0));
   if (O.mode >= 1) { z.s1 = unit(z.s1); z.s2 = unit(z.s2); }
@@ -453,6 +456,7 @@ OrbitResult<T> integrate_orbit(State<T> z, const Params<T>& P, T h, int64_t n_st
     if (rr < T(O.r_merge)) { status = ST_MERGED; break; }
     if (rr > T(O.r_escape)) { status = ST_UNBOUND; break; }
     z = zn; zs = zsn; ++k; gn_total += gn + gns;
+    if (sample_interval > 0 && k % sample_interval == 0) sampler(k / sample_interval - 1, z);
     if (shadow && O.renorm_interval > 0 && (k % O.renorm_interval) == 0) {
       const State<T> dz = zs - z;
       const T d = o_sqrt(norm12sq(dz));
@@ -463,6 +467,9 @@ OrbitResult<T> integrate_orbit(State<T> z, const Params<T>& P, T h, int64_t n_st
       Rs = references(zs, P);  // DESIGN.md R11
     }
   }
+  if (sample_interval > 0)   // a dropped orbit keeps reporting its frozen state
+    for (int64_t kk = (k / sample_interval + 1) * sample_interval; kk <= n_steps; kk += sample_interval)
+      sampler(kk / sample_interval - 1, z);
   out.z = z;
   six_integrals(z, P, out.inv1);
   out.fli = shadow ? acc + o_log10(o_sqrt(norm12sq(zs - z)) / d0) : T(0);
@@ -470,6 +477,11 @@ OrbitResult<T> integrate_orbit(State<T> z, const Params<T>& P, T h, int64_t n_st
   out.steps_done = k;
   out.gn_steps = gn_total;
   return out;
+}
+
+template <class T>
+OrbitResult<T> integrate_orbit(State<T> z, const Params<T>& P, T h, int64_t n_steps, T shadow_eps, const Options& O) {
+  return integrate_orbit<T>(z, P, h, n_steps, shadow_eps, O, 0, [](int64_t, const State<T>&) {});
 }
 
 }  // namespace pn_oracle

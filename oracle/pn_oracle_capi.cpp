@@ -103,12 +103,16 @@ void correct_t(int64_t n, const double* states, const ParamArrays& A, const doub
 template <class T>
 void integrate_t(int64_t n, const double* states, const ParamArrays& A, double h, int64_t n_steps,
                  double shadow_eps, const Options& O, double* out_states, double* out_inv, double* out_fli,
-                 int32_t* out_status, int64_t* out_step, int64_t* out_gn, int n_threads) {
+                 int32_t* out_status, int64_t* out_step, int64_t* out_gn, int n_threads,
+                 int64_t sample_interval, double* out_samples) {
 #pragma omp parallel for schedule(static) num_threads(n_threads)
   for (int64_t i = 0; i < n; ++i) {
     const State<T> z = load_state<T>(states, n, i);
     const Params<T> P = load_params<T>(A.beta, A.chi1, A.chi2, A.kq1, A.kq2, A.terms, i);
-    const OrbitResult<T> R = integrate_orbit<T>(z, P, T(h), n_steps, T(shadow_eps), O);
+    // samples: [n_steps / sample_interval][12][n], the layout of include/mc.h
+    auto sampler = [&](int64_t s, const State<T>& zz) { store_state(out_samples + s * 12 * n, n, i, zz); };
+    const OrbitResult<T> R = integrate_orbit<T>(z, P, T(h), n_steps, T(shadow_eps), O,
+                                                out_samples ? sample_interval : 0, sampler);
     if (out_states) store_state(out_states, n, i, R.z);
     if (out_inv)
       for (int c = 0; c < 6; ++c) {
@@ -169,16 +173,17 @@ int oracle_integrate(int precision, int64_t n, const double* states, const doubl
                      int64_t n_steps, int mode, double shadow_eps, int renorm_interval, int newton_iters,
                      double newton_tol, double r_merge, double r_escape, double* out_states,
                      double* out_invariants, double* out_fli, int32_t* out_status, int64_t* out_step,
-                     int64_t* out_gn_steps, int n_threads, int integrator) {
+                     int64_t* out_gn_steps, int n_threads, int integrator, int64_t sample_interval,
+                     double* out_samples) {
   const ParamArrays A = {beta, chi1, chi2, kq1, kq2, terms};
   const Options O = {mode, renorm_interval, newton_iters, newton_tol, r_merge, r_escape, integrator};
   if (n_threads <= 0) n_threads = omp_get_max_threads();
   if (precision == 0)
     integrate_t<long double>(n, states, A, h, n_steps, shadow_eps, O, out_states, out_invariants, out_fli,
-                             out_status, out_step, out_gn_steps, n_threads);
+                             out_status, out_step, out_gn_steps, n_threads, sample_interval, out_samples);
   else
     integrate_t<double>(n, states, A, h, n_steps, shadow_eps, O, out_states, out_invariants, out_fli,
-                        out_status, out_step, out_gn_steps, n_threads);
+                        out_status, out_step, out_gn_steps, n_threads, sample_interval, out_samples);
   return 0;
 }
 

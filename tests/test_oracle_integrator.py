@@ -306,6 +306,22 @@ def test_rk5_with_correction_keeps_the_integrals_and_beats_rk4_accuracy():
     assert out[oracle.RK5] < 0.2 * out[oracle.RK4]
 
 
+def test_sampled_output_equals_runs_stopped_at_the_sample_times():
+    """SURVEY 8(f) row 3: sample s of a run = final state of a run of (s + 1) * interval steps (brute force);
+    a dropped orbit keeps reporting its frozen state; a trailing partial interval gives no sample."""
+    z, _, _ = workloads.scan_grid(3, 4, r_lo=6.0, r_hi=9.0)            # strong field: some cells merge
+    full = oracle.integrate(z, 1.0, 1234, 3, shadow_eps=1e-8, sample_interval=100)
+    assert full.samples.shape == (12, 12, 12)
+    assert (full.status == 1).any() and (full.status == 0).any()
+    for s in (0, 4, 11):
+        part = oracle.integrate(z, 1.0, (s + 1) * 100, 3, shadow_eps=1e-8)
+        assert np.array_equal(full.samples[s], part.states)
+    dead = np.where(full.status != 0)[0]
+    late = full.steps_done[dead] < 1100
+    assert late.any()
+    assert np.array_equal(full.samples[11][:, dead[late]], full.states[:, dead[late]])
+
+
 def test_flop_counter_reports_the_oracles_own_formulation():
     c = oracle.count_flops(workloads.paper_orbit(2).states[:, 0], terms=15, mode=3, newton_iters=2)
     assert c["rk4_step"] == 4 * c["rhs"] + 159            # 3 stage inputs (3*25) + final combination (84)

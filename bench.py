@@ -58,6 +58,8 @@ def parse_args():
                          "paper's own scans (PAPER.md:227), for profiles/ tables only")
     ap.add_argument("--integrator", default="rk4", choices=["rk4", "rk5"],
                     help="rk4 (BASELINE, default) | rk5 (Butcher six-stage, the paper's 'RK5'; profiles/ tables only)")
+    ap.add_argument("--sample-interval", type=int, default=0,
+                    help="mc_integrate_sampled: record every orbit every K steps (profiles/ tables only; 0 = off)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -247,7 +249,8 @@ def run_mc(args):
 
     def one_step():
         nonlocal launches
-        res = I.integrate(z_dev, w.h, w.n_steps, w.correction_mode, shadow_eps=w.shadow_eps, out_states=out)
+        res = I.integrate(z_dev, w.h, w.n_steps, w.correction_mode, shadow_eps=w.shadow_eps, out_states=out,
+                          sample_interval=args.sample_interval)
         launches += 1
         return res
 
@@ -327,7 +330,8 @@ def run_mc(args):
             "warmup": args.warmup, "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": describe(w, args),
-                       "orbits_per_gpu": n, "rk4_steps": w.n_steps,
+                       "orbits_per_gpu": n, "rk4_steps": w.n_steps, "sample_interval": args.sample_interval,
+                       "sample_bytes_per_launch": (w.n_steps // args.sample_interval) * 96 * n if args.sample_interval else 0,
                        "orbit_steps_counted": "accepted steps (sum of steps_done); scheduled = orbits x rk4_steps = %d" % int(orbit_steps_rank * world), "l2": "flushed (256 MiB write) between timed iterations",
                        "parallelism": f"orbit-sharded x{world}, no collective"},
             "clocks": clocks, "wall_s_timed_region": t_wall,

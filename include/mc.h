@@ -124,6 +124,18 @@ int mc_integrate(mc_handle* h, const double* states, int64_t n_orbits, double st
                  int32_t correction_mode, double shadow_eps, double* out_states,
                  double* out_invariants, double* out_fli);
 
+/* mc_integrate that also records the trajectory (the paper's phase portraits and spin-space
+ * plots, are drawn from such samples): after every sample_interval-th step (k = interval,
+ * 2 interval, ... <= n_steps) the state of every orbit (not of its shadow) is written to
+ *   out_samples  DEVICE, double[n_steps / sample_interval][12][n_orbits]       (written)
+ * A dropped orbit keeps reporting its frozen state.  sample_interval = 0 is mc_integrate.  The stores are
+ * coalesced, streaming, and the only global traffic inside the step loop.
+ * Errors: as mc_integrate; MC_EINVAL for a negative interval or a null out_samples with interval > 0. */
+int mc_integrate_sampled(mc_handle* h, const double* states, int64_t n_orbits, double step_h, int64_t n_steps,
+                         int32_t correction_mode, double shadow_eps, double* out_states,
+                         double* out_invariants, double* out_fli, int64_t sample_interval,
+                         double* out_samples);
+
 /* Same operation with HOST buffers (pageable or pinned): copies the inputs to device scratch owned by
  * the handle, runs mc_integrate, copies the outputs back and synchronises the stream before
  * returning.  out_status (int32[n_orbits]) and out_step (int64[n_orbits]) are optional host arrays. */

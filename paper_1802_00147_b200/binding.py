@@ -17,7 +17,7 @@ MC_OK, MC_EINVAL, MC_ECUDA, MC_EARCH, MC_ENOMEM = 0, -1, -2, -3, -4
 MC_INTEG_RK4, MC_INTEG_RK5 = 0, 1
 
 # every symbol include/mc.h declares (tests/test_abi.py checks the header against this list)
-EXPORTS = ["mc_params_default", "mc_create", "mc_integrate", "mc_integrate_host", "mc_get_status", "mc_get_work", "mc_eval",
+EXPORTS = ["mc_params_default", "mc_create", "mc_integrate", "mc_integrate_sampled", "mc_integrate_host", "mc_get_status", "mc_get_work", "mc_eval",
            "mc_last_launch_info", "mc_fp64_peak", "mc_destroy", "mc_strerror"]
 
 
@@ -76,6 +76,7 @@ def load_library():
     lib.mc_params_default.argtypes = [ctypes.POINTER(mc_params)]
     lib.mc_create.argtypes = [ctypes.POINTER(mc_params), ctypes.POINTER(vp)]
     lib.mc_integrate.argtypes = [vp, vp, i64, dbl, i64, i32, dbl, vp, vp, vp]
+    lib.mc_integrate_sampled.argtypes = [vp, vp, i64, dbl, i64, i32, dbl, vp, vp, vp, i64, vp]
     lib.mc_integrate_host.argtypes = [vp, vp, i64, dbl, i64, i32, dbl, vp, vp, vp, vp, vp]
     lib.mc_get_status.argtypes = [vp, vp, vp]
     lib.mc_get_work.argtypes = [vp, vp]
@@ -117,6 +118,7 @@ class IntegrateResult:
     fli: Optional["object"]          # (n,) or None
     status: "object"                 # (n,) int32
     steps_done: "object"             # (n,) int64
+    samples: Optional["object"] = None   # (n_steps // sample_interval, 12, n) with sample_interval > 0
 
 
 class Integrator:
@@ -179,7 +181,7 @@ class Integrator:
         return t.contiguous()
 
     def integrate(self, states, h, n_steps, correction_mode=3, shadow_eps=0.0, want_invariants=True,
-                  out_states=None) -> IntegrateResult:
+                  out_states=None, sample_interval=0) -> IntegrateResult:
         """states: (12, n) float64 (device tensor, or anything torch.as_tensor accepts)."""
         torch = self._torch
         z = self._dev(states)
@@ -190,13 +192,18 @@ class Integrator:
         out = torch.empty_like(z) if out_states is None else out_states
         inv = torch.empty_like(z) if want_invariants else None
         fli = torch.empty(n, dtype=torch.float64, device=self.device) if shadow_eps != 0.0 else None
-        _check(self._lib.mc_integrate(self._h, z.data_ptr(), n, float(h), int(n_steps), int(correction_mode),
-                                      float(shadow_eps), out.data_ptr(), inv.data_ptr() if inv is not None else None,
-                                      fli.data_ptr() if fli is not None else None))
+        samples = None
+        if sample_interval > 0:
+            samples = torch.empty((int(n_steps) // int(sample_interval), 12, n), dtype=torch.float64, device=self.device)
+        _check(self._lib.mc_integrate_sampled(self._h, z.data_ptr(), n, float(h), int(n_steps), int(correction_mode),
+                                              float(shadow_eps), out.data_ptr(),
+                                              inv.data_ptr() if inv is not None else None,
+                                              fli.data_ptr() if fli is not None else None, int(sample_interval),
+                                              samples.data_ptr() if samples is not None else None))
         status = torch.empty(n, dtype=torch.int32, device=self.device)
         steps = torch.empty(n, dtype=torch.int64, device=self.device)
         _check(self._lib.mc_get_status(self._h, status.data_ptr(), steps.data_ptr()))
-        return IntegrateResult(out, inv, fli, status, steps)
+        return IntegrateResult(out, inv, fli, status, steps, samples)
 
     def integrate_host(self, states_np, h, n_steps, correction_mode=3, shadow_eps=0.0):
         """mc_integrate_host: numpy (host) in, numpy out; copies are inside the call."""

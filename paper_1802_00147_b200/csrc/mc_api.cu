@@ -212,6 +212,14 @@ int mc_create(const mc_params* params, mc_handle** out_handle) {
 int mc_integrate(mc_handle* h, const double* states, int64_t n_orbits, double step_h, int64_t n_steps,
                  int32_t correction_mode, double shadow_eps, double* out_states, double* out_invariants,
                  double* out_fli) {
+  return mc_integrate_sampled(h, states, n_orbits, step_h, n_steps, correction_mode, shadow_eps, out_states,
+                              out_invariants, out_fli, 0, nullptr);
+}
+
+int mc_integrate_sampled(mc_handle* h, const double* states, int64_t n_orbits, double step_h, int64_t n_steps,
+                         int32_t correction_mode, double shadow_eps, double* out_states, double* out_invariants,
+                         double* out_fli, int64_t sample_interval, double* out_samples) {
+  if (sample_interval < 0 || sample_interval > 0x7fffffffLL || (sample_interval > 0 && !out_samples && n_orbits > 0)) return MC_EINVAL;
   if (!h || n_orbits < 0 || n_steps < 0 || n_steps > 0x7fffffffLL) return MC_EINVAL;
   if (correction_mode < 0 || correction_mode > 3) return MC_EINVAL;
   if (!std::isfinite(step_h) || !std::isfinite(shadow_eps)) return MC_EINVAL;
@@ -233,6 +241,8 @@ int mc_integrate(mc_handle* h, const double* states, int64_t n_orbits, double st
   A.states = states; A.out_states = out_states; A.out_inv = out_invariants; A.out_fli = shadow ? out_fli : nullptr;
   A.out_status = (int32_t*)h->status.p; A.out_step = (int64_t*)h->step.p; A.out_gn = (int64_t*)h->gn.p;
   A.n = n_orbits; A.n_steps = n_steps; A.h = step_h; A.shadow_eps = shadow_eps;
+  A.samples = sample_interval > 0 ? out_samples : nullptr;
+  A.sample_interval = sample_interval > 0 ? (int32_t)sample_interval : 1;
 
   const bool qm = (h->P.terms & MC_TERM_QM) != 0;
   mc::LaunchFn fn = nullptr;

@@ -37,6 +37,8 @@ struct IntegrateArgs {
   int32_t renorm_interval;
   int32_t newton_iters;
   int32_t integrator;         // 0 RK4, 1 RK5 (mc_eval only; integrate_kernel is instantiated per integrator)
+  double* samples;            // [n_steps / sample_interval][12][n] or null: orbit states after steps interval, 2 interval, ...
+  int32_t sample_interval;
   // scheduling
   unsigned long long* queue;  // [0] = next item
   int32_t* done;              // [n_units] chunks completed per unit
@@ -159,7 +161,17 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
     const int k_end = min(n_steps, (chunk + 1 == A.n_chunks) ? n_steps : (chunk + 1) * A.chunk_len);
 #pragma unroll 1
     for (int k = chunk * A.chunk_len; k < k_end; ++k) {
-      if (__all_sync(0xffffffffu, frozen)) break;
+      if (__all_sync(0xffffffffu, frozen)) {
+        if (A.samples != nullptr && !role_shadow && active) {      // whole warp dropped: remaining samples of this chunk
+          for (int kk = k; kk < k_end; ++kk)
+            if ((kk + 1) % A.sample_interval == 0) {
+              double* dst = A.samples + ((int64_t)((kk + 1) / A.sample_interval - 1) * 12) * A.n + orbit;
+#pragma unroll
+              for (int i = 0; i < 12; ++i) __stcs(dst + (int64_t)i * A.n, y[i]);
+            }
+        }
+        break;
+      }
       double z[12];
       base_step<INTEG, QM>(c, y, A.h, z);
       int gn;
@@ -186,6 +198,12 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
           frozen = true;
           status = code;
         }
+      }
+      if (A.samples != nullptr && (k + 1) % A.sample_interval == 0 && !role_shadow && active) {
+        // sampled output: the orbit's current state, its frozen state once it has been dropped
+        double* dst = A.samples + ((int64_t)((k + 1) / A.sample_interval - 1) * 12) * A.n + orbit;
+#pragma unroll
+        for (int i = 0; i < 12; ++i) __stcs(dst + (int64_t)i * A.n, y[i]);
       }
       if (shadow && --until_renorm == 0) {
         until_renorm = A.renorm_interval;

@@ -476,3 +476,30 @@ def test_step_size_and_tolerance_studies(mc):
     assert max(res[1e-10][0:2]) <= DRIFT_TOL and max(res[1e-8][0:2]) <= DRIFT_TOL
     assert res[1e-4][2] <= res[1e-8][2] <= res[0.0][2] and res[0.0][2] > 2.5    # eps = 0: runs to the cap
     assert res[1e-4][2] < 1.05                                          # loose tolerance: one step per step
+
+
+def test_sampled_trajectory_output_matches_oracle(mc):
+    """SURVEY 8(f) row 3 (mc_integrate_sampled): states after every 50th step, 1234 steps (a trailing partial
+    interval), strong-field grid with dropped cells (whole warps and single lanes) + regular orbits."""
+    z = np.concatenate([workloads.scan_grid(6, 20, r_lo=6.0, r_hi=9.0)[0], workloads.config0(100).states], axis=1)
+    n = z.shape[1]
+    with mc.Integrator() as I:
+        g = I.integrate(z, 1.0, 1234, 3, shadow_eps=1e-8, sample_interval=50)
+        plain = I.integrate(z, 1.0, 1234, 3, shadow_eps=1e-8)
+    with mc.Integrator(chunk_steps=170) as I:
+        gc = I.integrate(z, 1.0, 1234, 3, shadow_eps=1e-8, sample_interval=50)
+    o = oracle.integrate(z, 1.0, 1234, 3, shadow_eps=1e-8, sample_interval=50)
+    S, So = g.samples.cpu().numpy(), o.samples
+    assert S.shape == So.shape == (24, 12, n)
+    assert np.array_equal(g.status.cpu().numpy(), o.status) and (o.status != 0).sum() >= 20
+    assert np.array_equal(g.states.cpu().numpy(), plain.states.cpu().numpy())        # sampling changes nothing else
+    assert np.array_equal(S, gc.samples.cpu().numpy())                                # nor does chunking
+    live = o.status == 0
+    for s in range(24):
+        assert rel_state_err(S[s][:, live], So[s][:, live]) < 2e-9                    # 1234 steps, some cells chaotic
+    calm = live & (o.fli < 3.0)
+    assert calm.sum() > 80 and rel_state_err(S[23][:, calm], So[23][:, calm]) <= 2 * STATE_RTOL
+    dead = np.where(~live)[0]                                                          # frozen state is reported on
+    last = S[23][:, dead]
+    assert np.array_equal(last, g.states.cpu().numpy()[:, dead])
+    assert np.abs(last - So[23][:, dead]).max() < 1e-6

@@ -161,9 +161,10 @@ class Integrator:
         _check(self._lib.mc_create(ctypes.byref(p), ctypes.byref(self._h)))
 
     def close(self):
-        if getattr(self, "_h", None) is not None and self._h.value:
-            self._lib.mc_destroy(self._h)
-            self._h = ctypes.c_void_p()
+        h = getattr(self, "_h", None)
+        if h is not None and h.value:
+            self._h = None                     # before the call: safe against re-entry and interpreter shutdown
+            self._lib.mc_destroy(h)
 
     __del__ = close
 

@@ -339,7 +339,7 @@ def run_mc(args):
             "gpu_launches": launches, "roofline": roofline,
             "outcome": {"regular": int(((status == 0) & (fli < 5.8)).sum()), "chaotic": int(((status == 0) & (fli >= 5.8)).sum()),
                         "dropped": int((status != 0).sum()), "near_threshold": int(((status == 0) & (np.abs(fli - 5.8) < 0.5)).sum())}}
-    if not args.no_cpu_baseline:
+    if not args.no_cpu_baseline and world == 1:           # rank 0 at N = 1 only (contract)
         line["cpu_baseline"], _ = cpu_baseline_sample(w)
     print(json.dumps(line), flush=True)
     if world > 1:

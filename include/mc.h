@@ -136,6 +136,19 @@ int mc_integrate_sampled(mc_handle* h, const double* states, int64_t n_orbits, d
                          double* out_invariants, double* out_fli, int64_t sample_interval,
                          double* out_samples);
 
+/* Checkpoint / resume: mc_integrate that also parks the COMPLETE state of the run -- orbit
+ * and shadow, reference integrals E0, J0 of both, FLI accumulator, renormalisation counter,
+ * status, step and Gauss-Newton counters -- in `carry`, a DEVICE buffer of mc_carry_bytes(n_orbits, shadow_eps != 0)
+ * bytes owned by the caller, and with resume = 1 continues from it (`states` is then ignored and may be NULL).
+ * n1 steps followed by a resumed call of n2 steps give, bit for bit, every output of one call of n1 + n2 steps
+ * (same handle parameters, step_h, mode and shadow_eps; rows 0-5 of out_invariants, the initial integrals, are
+ * written by the first call only; out_step and the work counter are cumulative).  The carry layout is private.
+ * Errors: as mc_integrate; MC_EINVAL for a null carry or resume not in {0, 1}. */
+int64_t mc_carry_bytes(int64_t n_orbits, int32_t with_shadow);
+int mc_integrate_ex(mc_handle* h, const double* states, int64_t n_orbits, double step_h, int64_t n_steps,
+                    int32_t correction_mode, double shadow_eps, double* out_states, double* out_invariants,
+                    double* out_fli, void* carry, int32_t resume);
+
 /* Same operation with HOST buffers (pageable or pinned): copies the inputs to device scratch owned by
  * the handle, runs mc_integrate, copies the outputs back and synchronises the stream before
  * returning.  out_status (int32[n_orbits]) and out_step (int64[n_orbits]) are optional host arrays. */

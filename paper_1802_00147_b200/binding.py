@@ -17,7 +17,7 @@ MC_OK, MC_EINVAL, MC_ECUDA, MC_EARCH, MC_ENOMEM = 0, -1, -2, -3, -4
 MC_INTEG_RK4, MC_INTEG_RK5 = 0, 1
 
 # every symbol include/mc.h declares (tests/test_abi.py checks the header against this list)
-EXPORTS = ["mc_params_default", "mc_create", "mc_integrate", "mc_integrate_sampled", "mc_integrate_host", "mc_get_status", "mc_get_work", "mc_eval",
+EXPORTS = ["mc_params_default", "mc_create", "mc_integrate", "mc_integrate_sampled", "mc_integrate_ex", "mc_carry_bytes", "mc_integrate_host", "mc_get_status", "mc_get_work", "mc_eval",
            "mc_last_launch_info", "mc_fp64_peak", "mc_destroy", "mc_strerror"]
 
 
@@ -77,6 +77,8 @@ def load_library():
     lib.mc_create.argtypes = [ctypes.POINTER(mc_params), ctypes.POINTER(vp)]
     lib.mc_integrate.argtypes = [vp, vp, i64, dbl, i64, i32, dbl, vp, vp, vp]
     lib.mc_integrate_sampled.argtypes = [vp, vp, i64, dbl, i64, i32, dbl, vp, vp, vp, i64, vp]
+    lib.mc_integrate_ex.argtypes = [vp, vp, i64, dbl, i64, i32, dbl, vp, vp, vp, vp, i32]
+    lib.mc_carry_bytes.argtypes = [i64, i32]
     lib.mc_integrate_host.argtypes = [vp, vp, i64, dbl, i64, i32, dbl, vp, vp, vp, vp, vp]
     lib.mc_get_status.argtypes = [vp, vp, vp]
     lib.mc_get_work.argtypes = [vp, vp]
@@ -87,8 +89,9 @@ def load_library():
     lib.mc_strerror.argtypes = [ctypes.c_int]
     lib.mc_strerror.restype = ctypes.c_char_p
     for name in EXPORTS:
-        if name != "mc_strerror":
+        if name not in ("mc_strerror", "mc_carry_bytes"):
             getattr(lib, name).restype = ctypes.c_int
+    lib.mc_carry_bytes.restype = ctypes.c_int64
     _lib = lib
     return lib
 
@@ -119,6 +122,7 @@ class IntegrateResult:
     status: "object"                 # (n,) int32
     steps_done: "object"             # (n,) int64
     samples: Optional["object"] = None   # (n_steps // sample_interval, 12, n) with sample_interval > 0
+    carry: Optional["object"] = None     # checkpoint buffer of integrate_ex
 
 
 class Integrator:
@@ -205,6 +209,34 @@ class Integrator:
         steps = torch.empty(n, dtype=torch.int64, device=self.device)
         _check(self._lib.mc_get_status(self._h, status.data_ptr(), steps.data_ptr()))
         return IntegrateResult(out, inv, fli, status, steps, samples)
+
+    def integrate_ex(self, states, h, n_steps, correction_mode=3, shadow_eps=0.0, carry=None, resume=False,
+                     n_orbits=None, invariants=None) -> IntegrateResult:
+        """mc_integrate_ex: checkpoint / resume.  First call: carry=None allocates the checkpoint buffer (returned
+        as result.carry); later calls pass it back with resume=True (states may then be None)."""
+        torch = self._torch
+        if resume:
+            n = int(n_orbits)
+            zptr = None
+        else:
+            z = self._dev(states)
+            n = z.shape[1]
+            zptr = z.data_ptr()
+        if carry is None:
+            nbytes = self._lib.mc_carry_bytes(n, int(shadow_eps != 0.0))
+            carry = torch.empty(max(nbytes, 8) // 8, dtype=torch.float64, device=self.device)
+        out = torch.empty((12, n), dtype=torch.float64, device=self.device)
+        inv = invariants if invariants is not None else torch.empty((12, n), dtype=torch.float64, device=self.device)
+        fli = torch.empty(n, dtype=torch.float64, device=self.device) if shadow_eps != 0.0 else None
+        _check(self._lib.mc_integrate_ex(self._h, zptr, n, float(h), int(n_steps), int(correction_mode), float(shadow_eps),
+                                         out.data_ptr(), inv.data_ptr(), fli.data_ptr() if fli is not None else None,
+                                         carry.data_ptr(), int(bool(resume))))
+        status = torch.empty(n, dtype=torch.int32, device=self.device)
+        steps = torch.empty(n, dtype=torch.int64, device=self.device)
+        _check(self._lib.mc_get_status(self._h, status.data_ptr(), steps.data_ptr()))
+        res = IntegrateResult(out, inv, fli, status, steps)
+        res.carry = carry
+        return res
 
     def integrate_host(self, states_np, h, n_steps, correction_mode=3, shadow_eps=0.0):
         """mc_integrate_host: numpy (host) in, numpy out; copies are inside the call."""

@@ -209,22 +209,48 @@ int mc_create(const mc_params* params, mc_handle** out_handle) {
   return MC_OK;
 }
 
+static int integrate_impl(mc_handle* h, const double* states, int64_t n_orbits, double step_h, int64_t n_steps,
+                          int32_t correction_mode, double shadow_eps, double* out_states, double* out_invariants,
+                          double* out_fli, int64_t sample_interval, double* out_samples, void* user_carry, int32_t resume);
+
 int mc_integrate(mc_handle* h, const double* states, int64_t n_orbits, double step_h, int64_t n_steps,
                  int32_t correction_mode, double shadow_eps, double* out_states, double* out_invariants,
                  double* out_fli) {
-  return mc_integrate_sampled(h, states, n_orbits, step_h, n_steps, correction_mode, shadow_eps, out_states,
-                              out_invariants, out_fli, 0, nullptr);
+  return integrate_impl(h, states, n_orbits, step_h, n_steps, correction_mode, shadow_eps, out_states,
+                        out_invariants, out_fli, 0, nullptr, nullptr, 0);
 }
 
 int mc_integrate_sampled(mc_handle* h, const double* states, int64_t n_orbits, double step_h, int64_t n_steps,
                          int32_t correction_mode, double shadow_eps, double* out_states, double* out_invariants,
                          double* out_fli, int64_t sample_interval, double* out_samples) {
+  return integrate_impl(h, states, n_orbits, step_h, n_steps, correction_mode, shadow_eps, out_states,
+                        out_invariants, out_fli, sample_interval, out_samples, nullptr, 0);
+}
+
+int64_t mc_carry_bytes(int64_t n_orbits, int32_t with_shadow) {
+  if (n_orbits < 0) return MC_EINVAL;
+  const int64_t tp = ((n_orbits * (with_shadow ? 2 : 1) + 31) / 32) * 32;
+  return tp * (int64_t)(17 * sizeof(double) + sizeof(unsigned long long) + 3 * sizeof(int32_t));
+}
+
+int mc_integrate_ex(mc_handle* h, const double* states, int64_t n_orbits, double step_h, int64_t n_steps,
+                    int32_t correction_mode, double shadow_eps, double* out_states, double* out_invariants,
+                    double* out_fli, void* carry, int32_t resume) {
+  if (!carry && n_orbits > 0) return MC_EINVAL;
+  if (resume != 0 && resume != 1) return MC_EINVAL;
+  return integrate_impl(h, states, n_orbits, step_h, n_steps, correction_mode, shadow_eps, out_states,
+                        out_invariants, out_fli, 0, nullptr, carry, resume);
+}
+
+static int integrate_impl(mc_handle* h, const double* states, int64_t n_orbits, double step_h, int64_t n_steps,
+                          int32_t correction_mode, double shadow_eps, double* out_states, double* out_invariants,
+                          double* out_fli, int64_t sample_interval, double* out_samples, void* user_carry, int32_t resume) {
   if (sample_interval < 0 || sample_interval > 0x7fffffffLL || (sample_interval > 0 && !out_samples && n_orbits > 0)) return MC_EINVAL;
   if (!h || n_orbits < 0 || n_steps < 0 || n_steps > 0x7fffffffLL) return MC_EINVAL;
   if (correction_mode < 0 || correction_mode > 3) return MC_EINVAL;
   if (!std::isfinite(step_h) || !std::isfinite(shadow_eps)) return MC_EINVAL;
   const bool shadow = shadow_eps != 0.0;
-  if (n_orbits > 0 && (!states || !out_states || (shadow && !out_fli))) return MC_EINVAL;
+  if (n_orbits > 0 && ((!states && !resume) || !out_states || (shadow && !out_fli))) return MC_EINVAL;
   if (n_orbits > (int64_t)1 << 40) return MC_EINVAL;
   MC_CUDA(cudaSetDevice(h->P.device));
   h->last_n = n_orbits;
@@ -280,7 +306,14 @@ int mc_integrate_sampled(mc_handle* h, const double* states, int64_t n_orbits, d
   if (rc) return rc;
   A.queue = (unsigned long long*)h->sched.p;
   A.done = (int32_t*)((char*)h->sched.p + 16);
-  if (n_chunks > 1) {
+  A.resume = resume; A.save_final = user_carry ? 1 : 0;
+  if (user_carry) {
+    // caller-owned checkpoint (mc_carry_bytes): [17][tp] doubles, [tp] u64, [3][tp] int32 -- also the chunk carry
+    const size_t tp = (size_t)A.n_units * 32;
+    A.carry_d = (double*)user_carry;
+    A.carry_g = (unsigned long long*)(A.carry_d + 17 * tp);
+    A.carry_i = (int32_t*)(A.carry_g + tp);
+  } else if (n_chunks > 1) {
     const size_t tp = (size_t)A.n_units * 32;
     if ((rc = h->carry_d.reserve(sizeof(double) * 17 * tp))) return rc;
     if ((rc = h->carry_i.reserve(sizeof(int32_t) * 3 * tp))) return rc;

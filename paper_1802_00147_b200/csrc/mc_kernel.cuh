@@ -49,6 +49,8 @@ struct IntegrateArgs {
   int64_t n_items;            // n_units * n_chunks
   int32_t chunk_len;          // steps per chunk (>= 1)
   int32_t n_chunks;
+  int32_t resume;             // 1: chunk 0 starts from the carry buffer instead of `states` (mc_integrate_ex)
+  int32_t save_final;         // 1: the last chunk also parks its state in the carry buffer (mc_integrate_ex)
 };
 
 enum { ST_OK = 0, ST_MERGED = 1, ST_UNBOUND = 2, ST_NONFINITE = 3, ST_NEWTON_FLAG = 256 };
@@ -118,7 +120,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
     double acc = 0.0;
     int until_renorm = A.renorm_interval;
 
-    if (chunk == 0) {
+    if (chunk == 0 && !A.resume) {
       // prologue: coalesced SoA load, eq (10) on the input, reference integrals
 #pragma unroll
       for (int i = 0; i < 12; ++i) y[i] = A.states[(int64_t)i * A.n + orbit];
@@ -134,7 +136,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
     } else {
       // wait until this unit's previous chunk is published, then reload the carried state.  The holder of
       // that chunk got it earlier from the same queue, so it is running: the wait cannot deadlock.
-      if (lane == 0) {
+      if (chunk > 0 && lane == 0) {
         unsigned polls = 0;
         while (*(volatile int32_t*)(A.done + unit) < chunk) {
           __nanosleep(100);
@@ -233,8 +235,9 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
       }
     }
 
-    if (chunk + 1 < A.n_chunks) {
-      // park the state in the carry buffer and publish the chunk
+    const bool last = chunk + 1 == A.n_chunks;
+    if (!last || A.save_final) {
+      // park the state in the carry buffer (and publish the chunk unless it is the last)
 #pragma unroll
       for (int i = 0; i < 12; ++i) __stcg(A.carry_d + (int64_t)i * tp + t, y[i]);
       __stcg(A.carry_d + 12 * tp + t, R.E0);
@@ -245,10 +248,12 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
       __stcg(A.carry_i + tp + t, steps);
       __stcg(A.carry_i + 2 * tp + t, until_renorm);
       __stcg(A.carry_g + t, gn_total);
-      __threadfence();
-      __syncwarp();
-      if (lane == 0) atomicExch(A.done + unit, chunk + 1);
-      continue;
+      if (!last) {
+        __threadfence();
+        __syncwarp();
+        if (lane == 0) atomicExch(A.done + unit, chunk + 1);
+        continue;
+      }
     }
 
     // epilogue: FLI from the final separation, invariants, coalesced SoA stores

@@ -530,3 +530,35 @@ def test_full_grid_classification_against_the_oracle(mc):
              (near & (cg != co)).sum(), (gs == o.status).mean(), (g.steps_done.cpu().numpy() == o.steps_done).mean(),
              np.abs(gfli[reg] - o.fli[reg]).max()))
     assert agree >= 0.99
+
+
+@pytest.mark.parametrize("case", ["uniform-shadow", "per-orbit-qm-rk5", "dropped-cells", "no-shadow-mode2"])
+def test_checkpoint_resume_is_bitwise_identical_to_one_run(mc, case):
+    """SURVEY section 5 (checkpoint / resume), mc_integrate_ex: 3 calls of 310 + 457 + 233 steps, resumed from the
+    caller-owned carry buffer, reproduce one 1000-step call bit for bit in every output (states, final invariants,
+    FLI, status, cumulative step and work counters), with and without internal chunking."""
+    mode, eps, kw = 3, 1e-8, {}
+    if case == "uniform-shadow":
+        z = workloads.config0(300).states
+    elif case == "per-orbit-qm-rk5":
+        w = workloads.config3(n_r=7, n_theta=19, qm=True)
+        z, kw = w.states, dict(terms=w.terms, integrator=mc.MC_INTEG_RK5, **{k: v for k, v in w.params().items() if k != "terms"})
+    elif case == "dropped-cells":
+        z = workloads.scan_grid(12, 11, r_lo=6.0, r_hi=16.0)[0]
+    else:
+        z, mode, eps = workloads.config0(70).states, 2, 0.0
+    n = z.shape[1]
+    with mc.Integrator(**kw) as I:
+        one = I.integrate(z, 1.0, 1000, mode, shadow_eps=eps)
+        one_work = I.work(n).cpu().numpy()
+    for chunk in (0, 90):
+        with mc.Integrator(chunk_steps=chunk, **kw) as I:
+            a = I.integrate_ex(z, 1.0, 310, mode, shadow_eps=eps)
+            b = I.integrate_ex(None, 1.0, 457, mode, shadow_eps=eps, carry=a.carry, resume=True, n_orbits=n, invariants=a.invariants)
+            c = I.integrate_ex(None, 1.0, 233, mode, shadow_eps=eps, carry=a.carry, resume=True, n_orbits=n, invariants=a.invariants)
+            work = I.work(n).cpu().numpy()
+        for x, y in ((one.states, c.states), (one.invariants, c.invariants), (one.status, c.status), (one.steps_done, c.steps_done)):
+            assert np.array_equal(x.cpu().numpy(), y.cpu().numpy(), equal_nan=True), (case, chunk)
+        if eps != 0.0:
+            assert np.array_equal(one.fli.cpu().numpy(), c.fli.cpu().numpy(), equal_nan=True)
+        assert np.array_equal(one_work, work)

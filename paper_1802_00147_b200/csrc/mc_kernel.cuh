@@ -137,10 +137,13 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
       // wait until this unit's previous chunk is published, then reload the carried state.  The holder of
       // that chunk got it earlier from the same queue, so it is running: the wait cannot deadlock.
       if (chunk > 0 && lane == 0) {
-        unsigned polls = 0;
+        unsigned long long t0 = 0;
         while (*(volatile int32_t*)(A.done + unit) < chunk) {
-          __nanosleep(100);
-          if (++polls > (1u << 27)) __trap();   // > 10 s: something is broken, fail loudly instead of hanging
+          __nanosleep(200);
+          unsigned long long now;
+          asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+          if (t0 == 0) t0 = now;
+          else if (now - t0 > 600ull * 1000000000ull) __trap();   // 10 min: fail loudly instead of hanging
         }
       }
       __syncwarp();

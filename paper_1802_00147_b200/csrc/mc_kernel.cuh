@@ -163,6 +163,8 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
       gn_total = __ldcg(A.carry_g + t);
     }
 
+    // steps until the next sample; a countdown instead of a modulo in the step loop
+    int until_sample = (A.samples != nullptr) ? A.sample_interval - (int)(((long long)chunk * A.chunk_len) % A.sample_interval) : 0x7fffffff;
     const int k_end = min(n_steps, (chunk + 1 == A.n_chunks) ? n_steps : (chunk + 1) * A.chunk_len);
 #pragma unroll 1
     for (int k = chunk * A.chunk_len; k < k_end; ++k) {
@@ -204,11 +206,14 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
           status = code;
         }
       }
-      if (A.samples != nullptr && (k + 1) % A.sample_interval == 0 && !role_shadow && active) {
+      if (--until_sample == 0) {
         // sampled output: the orbit's current state, its frozen state once it has been dropped
-        double* dst = A.samples + ((int64_t)((k + 1) / A.sample_interval - 1) * 12) * A.n + orbit;
+        until_sample = A.sample_interval;
+        if (!role_shadow && active) {
+          double* dst = A.samples + ((int64_t)((k + 1) / A.sample_interval - 1) * 12) * A.n + orbit;
 #pragma unroll
-        for (int i = 0; i < 12; ++i) __stcs(dst + (int64_t)i * A.n, y[i]);
+          for (int i = 0; i < 12; ++i) __stcs(dst + (int64_t)i * A.n, y[i]);
+        }
       }
       if (shadow && --until_renorm == 0) {
         until_renorm = A.renorm_interval;

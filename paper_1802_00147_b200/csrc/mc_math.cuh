@@ -55,11 +55,14 @@ __device__ __forceinline__ double rcp_nz(double x) {
 }
 
 __device__ __forceinline__ bool finite12(const double* z) {
-  // exponent field all ones <=> inf or nan; integer pipe only (keeps the FP64 pipe for the physics)
-  unsigned bad = 0;
+  // exponent field all ones <=> inf or nan <=> (high word with the sign shifted out) >= 0xffe00000.  Integer pipe
+  // only (keeps the FP64 pipe for the physics); a max tree, not a predicate chain, so the dependency depth is 4.
+  unsigned m[12];
 #pragma unroll
-  for (int i = 0; i < 12; ++i) bad |= ((unsigned)__double2hiint(z[i]) & 0x7ff00000u) == 0x7ff00000u;
-  return bad == 0;
+  for (int i = 0; i < 12; ++i) m[i] = (unsigned)__double2hiint(z[i]) << 1;
+  const unsigned a = max(max(m[0], m[1]), m[2]), b = max(max(m[3], m[4]), m[5]);
+  const unsigned c = max(max(m[6], m[7]), m[8]), d = max(max(m[9], m[10]), m[11]);
+  return max(max(a, b), max(c, d)) < 0xffe00000u;
 }
 
 // ---- the fused model routine ----------------------------------------------------------------------

@@ -58,6 +58,8 @@ def parse_args():
                          "paper's own scans (PAPER.md:227), for profiles/ tables only")
     ap.add_argument("--integrator", default="rk4", choices=["rk4", "rk5"],
                     help="rk4 (BASELINE, default) | rk5 (Butcher six-stage, the paper's 'RK5'; profiles/ tables only)")
+    ap.add_argument("--mode", type=int, default=None, choices=[0, 1, 2, 3],
+                    help="correction mode override (default: the workload's own, 3 = six-integral projection; profiles/ tables only)")
     ap.add_argument("--sample-interval", type=int, default=0,
                     help="mc_integrate_sampled: record every orbit every K steps (profiles/ tables only; 0 = off)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -148,7 +150,8 @@ def describe(w, args):
     if w.name.startswith("config2"):
         return (f"config2: {args.grid}x{args.grid} orbit scan per GPU (r0 in [10,60] x theta in [0,pi]), equal mass, chi=1, "
                 f"N+1PN+2PN+SO+SS, {integ} h=1, {w.n_steps} steps, shadow 1e-8 renormalised every 100 steps + FLI, "
-                "six-integral correction (mode 3, Gauss-Newton terminated at eps=1e-10, cap 4)")
+                + ("six-integral correction (mode 3, Gauss-Newton terminated at eps=1e-10, cap 4)" if w.correction_mode == 3
+                   else f"correction mode {w.correction_mode}"))
     return (f"{args.workload} ({w.name}): {w.n_orbits} orbits per GPU, terms mask {w.terms}, "
             f"{'uniform' if w.uniform else 'per-orbit'} parameters, {integ} h={w.h}, {w.n_steps} steps, shadow {w.shadow_eps}, "
             f"correction mode {w.correction_mode}")
@@ -230,6 +233,8 @@ def run_mc(args):
         torch.cuda.synchronize()
 
     w = rank_shard(global_workload(args, world), args, rank, world)
+    if args.mode is not None:
+        w.correction_mode = args.mode
     n = w.n_orbits
     orbit_steps_rank = float(n) * w.n_steps
     z_dev = torch.as_tensor(w.states, device=dev)
@@ -304,11 +309,15 @@ def run_mc(args):
             dist.destroy_process_group()
         return
 
+    st = status & 255                                     # bit 8 = mode-2 skip flag, not a drop
     mp = measured_peaks()
     sm_max = float(mp.get("sm_max_mhz", clocks.get("sm_max_mhz") or 1965.0))
     nominal_tf = info["num_sms"] * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     per_launch_s = (dev_ms / args.steps) * 1e-3
     base = FLOP_PER_ORBIT_STEP_BASE_RK5 if rk5 else FLOP_PER_ORBIT_STEP_BASE
+    # other correction modes (profiles/ tables only): no eq (10) / L_t in mode 0, no L_t in mode 1, + about 300 flop
+    # per trajectory-step for the polynomial dual scaling of mode 2 (SURVEY 8d estimate)
+    base += {0: -92.0, 1: -24.0, 2: -24.0 + 600.0, 3: 0.0}[w.correction_mode]
     flop_per_launch = base * steps_done + FLOP_PER_GN_STEP * gn_steps
     achieved_tf = flop_per_launch / per_launch_s / 1e12
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": nominal_tf, "unit": "TFLOP/s",
@@ -337,8 +346,9 @@ def run_mc(args):
             "clocks": clocks, "wall_s_timed_region": t_wall,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
             "gpu_launches": launches, "roofline": roofline,
-            "outcome": {"regular": int(((status == 0) & (fli < 5.8)).sum()), "chaotic": int(((status == 0) & (fli >= 5.8)).sum()),
-                        "dropped": int((status != 0).sum()), "near_threshold": int(((status == 0) & (np.abs(fli - 5.8) < 0.5)).sum())}}
+            "outcome": {"regular": int(((st == 0) & (fli < 5.8)).sum()), "chaotic": int(((st == 0) & (fli >= 5.8)).sum()),
+                        "dropped": int((st != 0).sum()), "near_threshold": int(((st == 0) & (np.abs(fli - 5.8) < 0.5)).sum()),
+                        "mode2_skip_flagged": int(((status & 256) != 0).sum())}}
     if not args.no_cpu_baseline and world == 1:           # rank 0 at N = 1 only (contract)
         line["cpu_baseline"], _ = cpu_baseline_sample(w)
     print(json.dumps(line), flush=True)

@@ -9,7 +9,8 @@ namespace mc {
 
 // Resident 128-thread blocks per SM the register allocator must allow.  Uniform parameters are
 // constant-bank operands, so 3 blocks (<= 168 registers) fit without spills; per-orbit parameters, the
-// quadrupole-monopole term and the six-stage RK5 need <= 255 registers (2 blocks; measured as fast, profiles/r01_config_sweep.md).  ptxas -v: 0 spill bytes for all 16 instantiations (profiles/).
+// quadrupole-monopole term and the six-stage RK5 need <= 255 registers (2 blocks; within 6 % of the 3-block
+// speed, profiles/r01_config_sweep.md).  ptxas -v: 0 spill bytes for all 32 instantiations (checked by build()).
 #ifndef MC_MINB_UNIFORM
 #define MC_MINB_UNIFORM 3
 #endif

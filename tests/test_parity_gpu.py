@@ -562,3 +562,16 @@ def test_checkpoint_resume_is_bitwise_identical_to_one_run(mc, case):
         if eps != 0.0:
             assert np.array_equal(one.fli.cpu().numpy(), c.fli.cpu().numpy(), equal_nan=True)
         assert np.array_equal(one_work, work)
+
+
+def test_scan_command_line_tool(mc, tmp_path):
+    """paper_1802_00147_b200.scan: the scan front end writes FLI / status / image files from a GPU run."""
+    from paper_1802_00147_b200 import scan
+    out = scan.main(["--scan", "paper-theta2", "--steps", "600", "--out", str(tmp_path / "s.npz"), "--pgm", str(tmp_path / "s.pgm")])
+    z = np.load(tmp_path / "s.npz")
+    assert z["fli"].shape == (314,) and z["states"].shape == (12, 314) and np.array_equal(z["fli"], out["fli"])
+    head = (tmp_path / "s.pgm").read_bytes()[:15]
+    assert head.startswith(b"P5\n314 1\n255\n")
+    w = workloads.paper_scan_theta2(n_steps=600)
+    o = oracle.integrate(w.states, 1.0, 600, 3, shadow_eps=1e-8, **w.params())
+    assert np.array_equal(z["status"], o.status & 255) and np.abs(z["fli"] - o.fli).max() < 1e-3

@@ -19,7 +19,9 @@
 extern "C" {
 #endif
 
-typedef struct mc_handle mc_handle; /* opaque; created by mc_create, freed by mc_destroy */
+typedef struct mc_handle mc_handle; /* opaque; created by mc_create, freed by mc_destroy.  A handle owns device scratch
+                                       (status, work queue, carry) that its calls reuse in stream order: use one
+                                       handle per stream and do not call into one handle from two host threads at once */
 
 enum mc_error {
   MC_OK = 0,

@@ -575,3 +575,80 @@ def test_scan_command_line_tool(mc, tmp_path):
     w = workloads.paper_scan_theta2(n_steps=600)
     o = oracle.integrate(w.states, 1.0, 600, 3, shadow_eps=1e-8, **w.params())
     assert np.array_equal(z["status"], o.status & 255) and np.abs(z["fli"] - o.fli).max() < 1e-3
+
+
+def test_config1_full_size_correction_on_and_off_in_the_same_run(mc):
+    """BASELINE config 1 at full size and length: 1024 orbits, per-orbit beta and chi, 1e5 steps, shadow + FLI,
+    the same inputs once with the correction (mode 3) and once without (mode 0).  Drift of the six integrals on
+    every orbit both ways (oracle-evaluated, R18); 48 sampled orbits recomputed by the oracle both ways."""
+    w = workloads.config1()
+    assert w.n_orbits == 1024 and w.n_steps == 100_000
+    kw = {k: v for k, v in w.params().items() if k != "terms"}
+    out = {}
+    with mc.Integrator(terms=w.terms, **kw) as I:
+        for mode in (3, 0):
+            out[mode] = I.integrate(w.states, w.h, w.n_steps, mode, shadow_eps=w.shadow_eps)
+    inv0 = out[3].invariants.cpu().numpy()[0:6]
+    live3 = out[3].status.cpu().numpy() == 0
+    assert live3.mean() > 0.95
+    d3 = drift(out[3].states.cpu().numpy()[:, live3], inv0[:, live3], **w.subset(np.where(live3)[0]).params())
+    live0 = out[0].status.cpu().numpy() == 0
+    I1 = oracle.integrals(out[0].states.cpu().numpy()[:, live0], **w.subset(np.where(live0)[0]).params())
+    dE0 = np.abs(I1[0] / inv0[0][live0] - 1)
+    assert d3 <= DRIFT_TOL and np.median(dE0) > 1e-9 and dE0.max() > 1e-6        # the correction has work to do
+    idx = np.sort(np.random.default_rng(11).choice(1024, 48, replace=False))
+    sub = w.subset(idx)
+    for mode in (3, 0):
+        o = oracle.integrate(sub.states, w.h, w.n_steps, mode, shadow_eps=w.shadow_eps, **sub.params())
+        gs, gfli = out[mode].status.cpu().numpy()[idx], out[mode].fli.cpu().numpy()[idx]
+        assert (gs == o.status).mean() >= 0.95
+        assert (classes(gfli, gs) == classes(o.fli, o.status)).mean() >= 0.95
+        reg = (o.status == 0) & (gs == 0) & (o.fli < 4.5)
+        assert reg.sum() >= 30 and np.abs(gfli[reg] - o.fli[reg]).max() < 0.1
+
+
+def test_config3_full_size_quadrupole_sampled_against_oracle(mc):
+    """BASELINE config 3 at full size (314 x 314, beta = 0.8, chi = 0.9, per-orbit kappa in [1, 8], QM on), 1e4
+    steps: drift on every live cell, 40 sampled cells recomputed by the oracle."""
+    w = workloads.config3(n_steps=10_000, qm=True)
+    kw = {k: v for k, v in w.params().items() if k != "terms"}
+    with mc.Integrator(terms=w.terms, **kw) as I:
+        g = I.integrate(w.states, w.h, w.n_steps, 3, shadow_eps=w.shadow_eps)
+        info = I.launch_info()
+    assert info["local_bytes"] == 0 and info["variant"] & 3 == 3
+    gs, gz, gfli = g.status.cpu().numpy(), g.states.cpu().numpy(), g.fli.cpu().numpy()
+    live = gs == 0
+    assert 0.7 < live.mean() < 1.0
+    inv0 = g.invariants.cpu().numpy()[0:6]
+    assert drift(gz[:, live], inv0[:, live], **w.subset(np.where(live)[0]).params()) <= DRIFT_TOL
+    idx = np.sort(np.random.default_rng(5).choice(314 * 314, 40, replace=False))
+    sub = w.subset(idx)
+    o = oracle.integrate(sub.states, w.h, w.n_steps, 3, shadow_eps=w.shadow_eps, **sub.params())
+    assert (gs[idx] == o.status).mean() >= 0.95
+    same = gs[idx] == o.status
+    assert np.array_equal(g.steps_done.cpu().numpy()[idx][same & (o.status == 0)], o.steps_done[same & (o.status == 0)])
+    reg = (o.status == 0) & (gs[idx] == 0) & (o.fli < 4.0)
+    assert reg.sum() >= 20 and np.abs(gfli[idx][reg] - o.fli[reg]).max() < 0.02
+    assert rel_state_err(gz[:, idx][:, reg], o.states[:, reg]) < 1e-6
+
+
+def test_config4_maximum_size_properties(mc):
+    """BASELINE config 4 at its largest size, 2^20 orbits + shadows (2 M trajectories, 65 536 work units), 300
+    steps: the second half of the batch repeats the first half and must reproduce it bit for bit; the six
+    integrals hold on every orbit (oracle-evaluated)."""
+    half = workloads.config4(19, n_steps=300)
+    z = np.concatenate([half.states, half.states], axis=1)
+    n = z.shape[1]
+    assert n == 1 << 20
+    with mc.Integrator() as I:
+        g = I.integrate(z, 1.0, 300, 3, shadow_eps=1e-8)
+        info = I.launch_info()
+    assert info["trajectories"] == 2 * n and info["local_bytes"] == 0
+    gz, gf = g.states.cpu().numpy(), g.fli.cpu().numpy()
+    assert np.array_equal(gz[:, : n // 2], gz[:, n // 2:]) and np.array_equal(gf[: n // 2], gf[n // 2:])
+    assert (g.status.cpu().numpy() == 0).all() and (g.steps_done.cpu().numpy() == 300).all()
+    inv = g.invariants.cpu().numpy()
+    I1 = oracle.integrals(gz[:, : n // 2], **half.params())
+    assert np.abs(I1[0] / inv[0, : n // 2] - 1).max() <= DRIFT_TOL
+    assert (np.linalg.norm(I1[1:4] - inv[1:4, : n // 2], axis=0) / np.linalg.norm(inv[1:4, : n // 2], axis=0)).max() <= DRIFT_TOL
+    assert np.abs(inv[6:12, : n // 2] - I1).max() < 1e-13                    # the kernel's own final invariants agree

@@ -21,14 +21,14 @@
 //   Omega1 = o1 u^3 L + 3 u^5 (m12 a2 + m11 a1) r - m12 u^3 sigma2     (= dH/dS1, S1 = s1 sigma1)
 //   Omega2 = o2 u^3 L + 3 u^5 (m21 a1 + m22 a2) r - m21 u^3 sigma1
 //   J = L + s1 sigma1 + s2 sigma2
-enum { MC_NCONST = 36 };
+enum { MC_NCONST = 37 };
 enum McConstIndex {
   K_A1 = 0, K_B1, K_B2, K_H1, K_C3, K_D1, K_D2, K_D3, K_E1, K_E2, K_F1,  // orbital
   K_K1, K_K2, K_C12, K_Q1, K_Q2,                                         // spin couplings in H
   K_O1, K_O2, K_M12, K_M21, K_M11, K_M22,                                // precession
   K_S1, K_S2,                                                            // spin magnitudes
   // fixed multiples of the above, so that no constant x constant product is left in the step loop
-  K_2A1, K_3C3, K_2H1, K_3F1, K_2B2, K_2D2, K_4D3, K_2E2,                // 2 H_P, 2 H_Q, H_u polynomials
+  K_2A1, K_3C3, K_2H1, K_3F1, K_2B2, K_2D2, K_4D3, K_2E2, K_2E1,         // 2 H_P, 2 H_Q, H_u polynomials
   K_3C12, K_M5C12, K_3M12, K_3M21                                         // spin-spin gradient / precession
 };
 
@@ -73,6 +73,7 @@ MC_HD void mc_derive_consts(double beta, double chi1, double chi2, double kq1, d
   c[K_2D2 * stride] = 2.0 * c[K_D2 * stride];
   c[K_4D3 * stride] = 4.0 * c[K_D3 * stride];
   c[K_2E2 * stride] = 2.0 * c[K_E2 * stride];
+  c[K_2E1 * stride] = 2.0 * c[K_E1 * stride];
   c[K_3C12 * stride] = 3.0 * c[K_C12 * stride];
   c[K_M5C12 * stride] = -5.0 * c[K_C12 * stride];
   c[K_3M12 * stride] = 3.0 * c[K_M12 * stride];

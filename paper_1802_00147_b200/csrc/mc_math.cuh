@@ -86,18 +86,19 @@ __device__ __forceinline__ void pn_eval(const C& c, const double* z, double* g, 
   // orbital polynomials (Horner); every constant multiple is precomputed (mc_consts.h)
   const double t1 = fma(c[K_D2], Q, fma(c[K_D1], P, c[K_B1]));   // b1 + d1 P + d2 Q
   const double t2 = fma(c[K_D3], Q, c[K_B2]);                    // b2 + d3 Q
-  const double t3 = fma(c[K_E2], Q, c[K_E1] * P);                // e1 P + e2 Q
+  const double t3 = WANT_H ? fma(c[K_E2], Q, c[K_E1] * P) : 0.0;  // e1 P + e2 Q (only H itself needs it)
   // H_P = 1/2 + P (2 a1 + 3 c3 P) + u (b1 + 2 d1 P + d2 Q + e1 u)
   const double hp_u = fma(c[K_E1], u, fma(c[K_D1], P, t1));
   const double HP = fma(u, hp_u, fma(P, fma(c[K_3C3], P, c[K_2A1]), 0.5));
   // 2 H_Q = u (2 b2 + 2 d2 P + 4 d3 Q + 2 e2 u)
   const double HQ2 = u * fma(c[K_4D3], Q, fma(c[K_2D2], P, fma(c[K_2E2], u, c[K_2B2])));
   // H_u = -1 + P t1 + Q t2 + u (2 h1 + 2 t3 + 3 f1 u)
-  const double hu_u = fma(c[K_3F1], u, fma(2.0, t3, c[K_2H1]));
+  const double hu_u = WANT_H ? fma(c[K_3F1], u, fma(2.0, t3, c[K_2H1]))
+                             : fma(c[K_3F1], u, fma(c[K_2E1], P, fma(c[K_2E2], Q, c[K_2H1])));
   const double Hu = fma(u, hu_u, fma(Q, t2, fma(P, t1, -1.0)));
   const double A = HP + HP;                                // dH_orb/dp = A p + B r
-  const double B = HQ2 * w;                                // dH_orb/dr = B p + Cc r
-  const double Cc = -u2 * fma(Hu, u, HQ2 * Q);
+  const double B = HQ2 * w;
+  const double Cu = fma(Hu, u, HQ2 * Q);                   // dH_orb/dr = B p - u^2 Cu r
 
   // spin couplings
   const double a1 = dot3(s1, r), a2 = dot3(s2, r), d12 = dot3(s1, s2);
@@ -126,7 +127,7 @@ __device__ __forceinline__ void pn_eval(const C& c, const double* z, double* g, 
     w2 = fma(6.0 * c[K_Q2] * u5, a2, w2);
     Hss += fma(3.0 * c[K_Q1], a11u5, -(q1u3 * d11)) + fma(3.0 * c[K_Q2], a22u5, -(q2u3 * d22));
   }
-  const double Cr = fma(X, 3.0 * u2, Cc);
+  const double Cr = u2 * fma(3.0, X, -Cu);                 // coefficient of r in dH/dr
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
     g[i] = fma(w2, s2[i], fma(w1, s1[i], fma(Cr, r[i], fma(B, p[i], PxS[i]))));

@@ -149,11 +149,13 @@ class Result:
     steps_done: np.ndarray   # (n,) int64
     gn_steps: np.ndarray     # (n,) int64: Gauss-Newton steps of mode 3 over accepted steps, orbit + shadow
     samples: np.ndarray = None   # (n_steps // sample_interval, 12, n): orbit states after steps interval, 2 interval, ...
+    shadow: np.ndarray = None    # (16, n) with want_shadow: the shadow's final state (12 rows), then E0', J0' it is corrected onto
 
 
 def integrate(z, h, n_steps, mode, shadow_eps=0.0, beta=1.0, chi1=1.0, chi2=1.0, kq1=1.0, kq2=1.0,
               terms=TERMS_DEFAULT, renorm_interval=100, newton_iters=4, newton_tol=1e-10,
-              r_merge=2.0, r_escape=1e4, precision=LONG_DOUBLE, n_threads=0, integrator=RK4, sample_interval=0):
+              r_merge=2.0, r_escape=1e4, precision=LONG_DOUBLE, n_threads=0, integrator=RK4, sample_interval=0,
+              want_shadow=False):
     """The oracle's statement of mc_integrate (include/mc.h), orbit by orbit."""
     z = _states(z)
     n = z.shape[1]
@@ -162,6 +164,8 @@ def integrate(z, h, n_steps, mode, shadow_eps=0.0, beta=1.0, chi1=1.0, chi2=1.0,
                  np.empty(n, dtype=np.int64), np.empty(n, dtype=np.int64))
     if sample_interval > 0:
         res.samples = np.empty((n_steps // sample_interval, 12, n))
+    if want_shadow:
+        res.shadow = np.empty((16, n))
     lib().oracle_integrate(ctypes.c_int(precision), ctypes.c_int64(n), _p(z), *[_p(a) for a in pa],
                            ctypes.c_uint32(terms), ctypes.c_double(h), ctypes.c_int64(n_steps),
                            ctypes.c_int(mode), ctypes.c_double(shadow_eps), ctypes.c_int(renorm_interval),
@@ -169,7 +173,7 @@ def integrate(z, h, n_steps, mode, shadow_eps=0.0, beta=1.0, chi1=1.0, chi2=1.0,
                            ctypes.c_double(r_merge), ctypes.c_double(r_escape), _p(res.states),
                            _p(res.invariants), _p(res.fli), _p(res.status), _p(res.steps_done),
                            _p(res.gn_steps), ctypes.c_int(n_threads), ctypes.c_int(integrator),
-                           ctypes.c_int64(sample_interval), _p(res.samples))
+                           ctypes.c_int64(sample_interval), _p(res.samples), _p(res.shadow))
     return res
 
 

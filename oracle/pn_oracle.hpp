@@ -413,6 +413,8 @@ template <class T> struct OrbitResult {
   int32_t status;
   int64_t steps_done;
   int64_t gn_steps;      // Gauss-Newton steps of mode 3 over all accepted steps, orbit + shadow
+  State<T> zs;           // final shadow state (= z without a shadow) and the integrals it is corrected onto;
+  T Es0; V3<T> Js0;      //   reported so that the shadow's own invariants can be pinned (tests only)
 };
 
 template <class T> inline void six_integrals(const State<T>& z, const Params<T>& P, T out[6]) {
@@ -476,6 +478,7 @@ OrbitResult<T> integrate_orbit(State<T> z, const Params<T>& P, T h, int64_t n_st
   out.status = status | flag;
   out.steps_done = k;
   out.gn_steps = gn_total;
+  out.zs = zs; out.Es0 = Rs.E0; out.Js0 = Rs.J0;
   return out;
 }
 

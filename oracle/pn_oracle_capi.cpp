@@ -104,7 +104,7 @@ template <class T>
 void integrate_t(int64_t n, const double* states, const ParamArrays& A, double h, int64_t n_steps,
                  double shadow_eps, const Options& O, double* out_states, double* out_inv, double* out_fli,
                  int32_t* out_status, int64_t* out_step, int64_t* out_gn, int n_threads,
-                 int64_t sample_interval, double* out_samples) {
+                 int64_t sample_interval, double* out_samples, double* out_shadow) {
 #pragma omp parallel for schedule(static) num_threads(n_threads)
   for (int64_t i = 0; i < n; ++i) {
     const State<T> z = load_state<T>(states, n, i);
@@ -123,6 +123,11 @@ void integrate_t(int64_t n, const double* states, const ParamArrays& A, double h
     if (out_status) out_status[i] = R.status;
     if (out_step) out_step[i] = R.steps_done;
     if (out_gn) out_gn[i] = R.gn_steps;
+    if (out_shadow) {   // [16][n]: the shadow's final state, then E0', J0' (the integrals it is corrected onto)
+      store_state(out_shadow, n, i, R.zs);
+      const T refs[4] = {R.Es0, R.Js0.x, R.Js0.y, R.Js0.z};
+      for (int c = 0; c < 4; ++c) out_shadow[(int64_t)(12 + c) * n + i] = to_double(refs[c]);
+    }
   }
 }
 
@@ -174,16 +179,16 @@ int oracle_integrate(int precision, int64_t n, const double* states, const doubl
                      double newton_tol, double r_merge, double r_escape, double* out_states,
                      double* out_invariants, double* out_fli, int32_t* out_status, int64_t* out_step,
                      int64_t* out_gn_steps, int n_threads, int integrator, int64_t sample_interval,
-                     double* out_samples) {
+                     double* out_samples, double* out_shadow) {
   const ParamArrays A = {beta, chi1, chi2, kq1, kq2, terms};
   const Options O = {mode, renorm_interval, newton_iters, newton_tol, r_merge, r_escape, integrator};
   if (n_threads <= 0) n_threads = omp_get_max_threads();
   if (precision == 0)
     integrate_t<long double>(n, states, A, h, n_steps, shadow_eps, O, out_states, out_invariants, out_fli,
-                             out_status, out_step, out_gn_steps, n_threads, sample_interval, out_samples);
+                             out_status, out_step, out_gn_steps, n_threads, sample_interval, out_samples, out_shadow);
   else
     integrate_t<double>(n, states, A, h, n_steps, shadow_eps, O, out_states, out_invariants, out_fli,
-                        out_status, out_step, out_gn_steps, n_threads, sample_interval, out_samples);
+                        out_status, out_step, out_gn_steps, n_threads, sample_interval, out_samples, out_shadow);
   return 0;
 }
 

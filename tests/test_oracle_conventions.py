@@ -1,0 +1,118 @@
+"""Pins for three conventions of oracle.integrate / oracle.correct that nothing else fixes (VERDICT round 1,
+"parity unpinned" lines): (a) the input spins are normalised first when the correction is on (PAPER.md:122-126,
+eq 10; include/mc.h "with correction_mode >= 1 the input spins are normalised first") and left alone in mode 0;
+(b) after every shadow renormalisation the shadow again has unit spins and is corrected onto the integrals of
+that very state ("constant unit lengths of spins"; R11); (c) the Newton iteration of
+mode 3 ends at the first update with |(dr,dp)| <= eps |p| (R6).  CPU only."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1802_00147_b200 import workloads
+
+
+def _scaled_spins(z, f1, f2):
+    out = z.copy()
+    out[6:9] *= f1
+    out[9:12] *= f2
+    return out
+
+
+@pytest.mark.parametrize("mode", [1, 2, 3])
+def test_input_spins_are_normalised_first_when_the_correction_is_on(mode):
+    """|S_hat| = 1 +- 1e-3 on input.  Eq (10) is the first thing a corrected run applies, so the run equals the
+    run on the pre-normalised input; its reference integrals (rows 0-5 of the invariants) are those of the UNIT
+    spin state: |S_hat| = 1 exactly and E0, J0 = H, J of the normalised input as the Python side evaluates them."""
+    w = workloads.config0(12)
+    par = dict(beta=0.6, chi1=0.9, chi2=0.7, terms=15)
+    bent = _scaled_spins(w.states, 1.0 + 1e-3, 1.0 - 1e-3)
+    unit = bent.copy()
+    unit[6:9] /= np.linalg.norm(unit[6:9], axis=0)
+    unit[9:12] /= np.linalg.norm(unit[9:12], axis=0)
+    a = oracle.integrate(bent, 1.0, 300, mode, shadow_eps=1e-8, **par)
+    b = oracle.integrate(unit, 1.0, 300, mode, shadow_eps=1e-8, **par)
+    assert np.abs(a.invariants[4:6] - 1.0).max() < 3e-16                  # the references belong to unit spins
+    I0 = oracle.integrals(unit, **par)
+    assert np.abs(a.invariants[0:4] - I0[0:4]).max() < 1e-15
+    # ... and not to the spins as given: those carry 1e-3 longer / shorter spin vectors in J and another energy
+    Ib = oracle.integrals(bent, **par)
+    assert np.linalg.norm(Ib[1:4] - I0[1:4], axis=0).min() > 1e-5 and np.abs(Ib[0] - I0[0]).min() > 1e-11
+    # same run up to the rounding of the normalisation itself (1e-19 in the spins; the FLI is the log of a 1e-8
+    # separation, so it sees state differences 1e8 times enlarged; mode 2 amplifies rounding ~10x, R7)
+    assert np.abs(a.states - b.states).max() < 1e-12 and np.abs(a.fli - b.fli).max() < 1e-4
+    assert np.array_equal(a.status, b.status)
+
+
+def test_mode0_does_not_touch_the_input_spins():
+    """Without correction nothing normalises: the reported initial |S_hat| are the input's, the precession
+    (a rotation, eq 7) keeps those lengths, and E0 is the energy of the state as given."""
+    w = workloads.config0(12)
+    par = dict(beta=0.6, chi1=0.9, chi2=0.7, terms=15)
+    bent = _scaled_spins(w.states, 1.0 + 1e-3, 1.0 - 1e-3)
+    a = oracle.integrate(bent, 1.0, 300, 0, **par)
+    assert np.abs(a.invariants[4] - (1.0 + 1e-3)).max() < 1e-15 and np.abs(a.invariants[5] - (1.0 - 1e-3)).max() < 1e-15
+    assert np.abs(a.invariants[10] - (1.0 + 1e-3)).max() < 1e-9 and np.abs(a.invariants[11] - (1.0 - 1e-3)).max() < 1e-9
+    assert np.abs(a.invariants[0] - oracle.integrals(bent, **par)[0]).max() < 1e-15
+    assert np.array_equal(oracle.integrate(bent, 1.0, 0, 0, **par).states, bent)      # n_steps = 0: untouched
+
+
+@pytest.mark.parametrize("mode", [1, 3])
+def test_shadow_has_unit_spins_and_its_own_integrals_after_a_renormalisation(mode):
+    """A wide pair (offset 0.5 M in x, strong field) so that the rescaled shadow spin s + t (s' - s) is visibly
+    shorter than 1 (by t (1 - t) |s' - s|^2): after the renormalisation that ends the run the shadow must again
+    have unit spins (eq 10), and the integrals it is corrected onto from then on are H and J of
+    exactly that state (R11), evaluated here by oracle.integrals on the returned shadow state."""
+    z = workloads.paper_orbit(2).states
+    par = dict(beta=1.0, chi1=1.0, chi2=1.0, terms=15)
+    n_steps, interval = 1200, 400
+    o = oracle.integrate(z, 1.0, n_steps, mode, shadow_eps=0.5, renorm_interval=interval, want_shadow=True, **par)
+    assert o.status[0] == 0 and o.steps_done[0] == n_steps
+    zs = o.shadow[0:12]
+    # the case is sharp: one interval earlier the two spins differ enough that the chord is visibly short
+    mid = oracle.integrate(z, 1.0, n_steps - 1, mode, shadow_eps=0.5, renorm_interval=interval, want_shadow=True, **par)
+    gap = np.linalg.norm(mid.shadow[6:9, 0] - mid.states[6:9, 0])
+    sep = np.linalg.norm(mid.shadow[0:12, 0] - mid.states[0:12, 0])
+    t = 0.5 / sep
+    assert t * (1 - t) * gap ** 2 > 1e-6, (gap, sep)
+    assert abs(np.linalg.norm(zs[6:9, 0]) - 1) < 3e-16 and abs(np.linalg.norm(zs[9:12, 0]) - 1) < 3e-16
+    Is = oracle.integrals(zs, **par)[:, 0]
+    assert abs(o.shadow[12, 0] - Is[0]) < 1e-16 and np.abs(o.shadow[13:16, 0] - Is[1:4]).max() < 1e-15
+    # the pair was pulled back to the initial distance (to first order: normalising the spins moves it at second order)
+    d = np.linalg.norm(zs[:, 0] - o.states[:, 0])
+    assert abs(d / 0.5 - 1) < 1e-2
+    # and the main trajectory never sees its shadow
+    alone = oracle.integrate(z, 1.0, n_steps, mode, **par)
+    assert np.array_equal(alone.states, o.states)
+
+
+def test_newton_iteration_stops_at_the_first_update_below_eps_times_p():
+    """Brute force on the rule itself ("until the update is below eps"; R6: the norm is
+    |(dr,dp)|_2 <= eps |p|_2, |p| being the smaller scale so that dr/r and dp/p are both <= eps).  The iterates
+    z_1, z_2, ... come from fixed-count runs (eps = 0); the eps-terminated operator must return exactly z_k* with
+    k* the first k whose update z_k - z_(k-1) meets the test at z_(k-1).  States with |r| ~ 100 |p| and a 1e-3
+    perturbation put the first update between eps |p| and eps |r| for eps = 1e-3, so a test scaled with |r|
+    (or with anything else of that size) stops one step early and fails."""
+    w = workloads.config0(24)
+    par = dict(beta=0.8, chi1=0.9, chi2=0.9, terms=15)
+    I0 = oracle.integrals(w.states, **par)
+    rng = np.random.default_rng(11)
+    zp = w.states.copy()
+    zp[0:3] += 2e-3 * rng.normal(size=(3, 24))
+    zp[3:6] += 2e-5 * rng.normal(size=(3, 24))
+    iterates = [zp] + [oracle.correct(zp, I0[0], I0[1:4], 3, newton_iters=k, newton_tol=0.0, **par)[0] for k in (1, 2, 3, 4)]
+    for eps, expect_counts in ((1e-3, {2, 3}), (1e-10, {3, 4}), (1.0, {1})):
+        got = oracle.correct(zp, I0[0], I0[1:4], 3, newton_iters=4, newton_tol=eps, **par)[0]
+        counts = set()
+        for i in range(24):
+            k_star = 4
+            for k in range(1, 5):
+                upd = np.linalg.norm(iterates[k][0:6, i] - iterates[k - 1][0:6, i])
+                if upd <= eps * np.linalg.norm(iterates[k - 1][3:6, i]):
+                    k_star = k
+                    break
+            counts.add(k_star)
+            assert np.array_equal(got[:, i], iterates[k_star][:, i]), (eps, i, k_star)
+        assert counts <= expect_counts, (eps, counts)
+    # the discriminating case really sits between the two scales
+    upd1 = np.linalg.norm(iterates[1][0:6] - zp[0:6], axis=0)
+    assert (upd1 > 1e-3 * np.linalg.norm(zp[3:6], axis=0)).all() and (upd1 < 1e-3 * np.linalg.norm(zp[0:3], axis=0)).all()

@@ -216,11 +216,42 @@ def test_mode2_dual_scaling_parity_on_unskipped_orbits(mc):
     # from its long-double instance by median 1.5e-12 / p90 6.7e-12 / max 4.0e-10 on this very input
     # (tests/test_oracle_integrator.py::test_mode2_rounding_amplification_sets_the_parity_bound), i.e.
     # ~10x the mode-3 figure.  The kernel must sit within the same envelope.
-    assert np.median(per_orbit) <= 1e-11 and np.quantile(per_orbit, 0.9) <= 1e-10 and per_orbit.max() <= 1e-8
+    # Round 2: bounds at ~3x what the kernel measures (1.4e-12 / 5.8e-12 / 1.6e-10), inside the oracle's own envelope.
+    assert np.median(per_orbit) <= 5e-12 and np.quantile(per_orbit, 0.9) <= 2e-11 and per_orbit.max() <= 5e-10
     I1 = oracle.integrals(g.states.cpu().numpy()[:, clean], **w.subset(np.where(clean)[0]).params())
     I0 = o.invariants[0:6, clean]
     assert np.abs(I1[0] / I0[0] - 1).max() < DRIFT_TOL
     assert np.abs(np.linalg.norm(I1[1:4], axis=0) / np.linalg.norm(I0[1:4], axis=0) - 1).max() < DRIFT_TOL
+
+
+@pytest.mark.parametrize("mode", [0, 1, 2, 3])
+def test_non_unit_input_spins(mc, mode):
+    """include/mc.h: "with correction_mode >= 1 the input spins are normalised first" (eq 10, PAPER.md:122-126);
+    mode 0 leaves them alone.  Input |S_hat| = 1 +- 1e-3, per-orbit parameters, shadow on, 150 orbits (ragged
+    tail).  The oracle side of this convention is pinned in tests/test_oracle_conventions.py."""
+    w = workloads.config1().subset(np.arange(150))
+    bent = w.states.copy()
+    bent[6:9] *= 1.0 + 1e-3
+    bent[9:12] *= 1.0 - 1e-3
+    kw = {k: v for k, v in w.params().items() if k != "terms"}
+    with mc.Integrator(terms=w.terms, **kw) as I:
+        g = I.integrate(bent, 1.0, 500, mode, shadow_eps=1e-8)
+    o = oracle.integrate(bent, 1.0, 500, mode, shadow_eps=1e-8, **w.params())
+    gz, ginv, gs = g.states.cpu().numpy(), g.invariants.cpu().numpy(), g.status.cpu().numpy()
+    assert np.abs(ginv[0:6] - o.invariants[0:6]).max() < 1e-14           # reference integrals of the same state
+    if mode == 0:
+        assert np.abs(ginv[4] - (1 + 1e-3)).max() < 1e-15 and np.abs(ginv[5] - (1 - 1e-3)).max() < 1e-15
+        assert np.abs(np.linalg.norm(gz[6:9], axis=0) - (1 + 1e-3)).max() < 1e-8    # RK4 keeps the length it was given
+    else:
+        assert np.abs(ginv[4:6] - 1).max() < 3e-16
+        assert np.abs(np.linalg.norm(gz[6:9], axis=0) - 1).max() < 3e-16
+    clean = (o.status == 0) & (gs == 0)                                   # mode 2: orbits with no skipped step (R7)
+    assert clean.sum() >= (30 if mode == 2 else 150)
+    if mode != 2:
+        assert np.array_equal(gs, o.status)
+    err = rel_state_err(gz[:, clean], o.states[:, clean])
+    assert err <= (5e-10 if mode == 2 else STATE_RTOL), err
+    assert np.abs(g.fli.cpu().numpy()[clean] - o.fli[clean]).max() < (1e-2 if mode == 2 else 1e-3)
 
 
 def test_batch_properties(mc):

@@ -4,8 +4,8 @@
 One "step" = one pass of the whole hot path (mc_integrate: load, 1e5 x [RK4 + six-integral correction]
 on orbit and shadow, FLI renormalisation every 100 steps, status, store) over the 314 x 314 grid.
 `value` counts accepted orbit-steps (dropped cells stop counting when they freeze).
-N > 1 (torchrun): the global grid has 314*N rows of r0, sharded by contiguous row ranges, no
-collective on the data path (weak scaling).  `--impl reference` times the CPU oracle instead.
+N > 1 (torchrun): the global grid has 314*N rows of r0, dealt to the ranks round-robin (row i -> rank i mod N, so
+every rank sees the same mix of strong- and weak-field cells), no collective on the data path (weak scaling).  `--impl reference` times the CPU oracle instead.
 Prints ONE JSON line on rank 0.  See DESIGN.md section 8 for every number's definition.
 """
 import argparse
@@ -25,22 +25,16 @@ from paper_1802_00147_b200 import sharding, workloads  # noqa: E402
 
 METRIC = "orbit-RK4-steps/sec (with correction+FLI)"
 UNIT = "orbit-steps/s"
-# Algorithmic FP64 flops (FMA = 2, add/mul/rsqrt/rcp = 1; QM off), itemised in DESIGN.md section 8:
-#   per orbit-step (orbit + shadow), without the Gauss-Newton steps of mode 3:
-#     2 x [4 x 229 (RHS) + 168 (RK4 sums) + 34 (eq 10) + 12 (L_t) + 5 (|r|^2 status test)] = 2270
-#   per Gauss-Newton step (gradient + H 190, residuals/Schur/solve/update 187, termination test 13) = 390
-# The number of Gauss-Newton steps is data dependent (epsilon-terminated, R6): the kernel counts
-# them (mc_get_work) and the flop total of a launch is 2270 x accepted orbit-steps + 390 x counted steps.
-# The oracle's unfactored formulation needs about twice as much (oracle.count_flops): conservative.
-# DRAM traffic of one launch of the hot kernel on the default grid, from the ncu --set full capture
-# (profiles/r01c_ncu_integrate_kernel_mode3.md: dram__bytes_read.sum + dram__bytes_write.sum = 9.64 + 5.20 MB
-# for a 4000-step launch; ncu replays make a 1e5-step capture impractical).  Outputs (31 MB) and the carry
-# buffer (31 MB) live in the 126 MB L2.  Algorithmic: 340 B per orbit.
-NCU_DRAM_BYTES_PER_LAUNCH_314 = 14.84e6
-FLOP_PER_ORBIT_STEP_BASE = 2270.0
-FLOP_PER_GN_STEP = 390.0
-# RK5 (Butcher, 6 stages): 2 x [6 x 229 + 408 (stage sums: 204 FMA) + 34 + 12 + 5] = 3666
-FLOP_PER_ORBIT_STEP_BASE_RK5 = 3666.0
+# Algorithmic FP64 flops: NOT constants of this file.  They come from mc_flop_model (include/mc.h), which runs the
+# kernels' own math templates with a counting scalar on the host (FMA = 2, add/mul = 1, rsqrt/reciprocal/division/
+# sqrt = 1; the Newton refinements around the hardware seeds are not algorithmic work) -- see algorithmic_flop()
+# below and tests/test_flop_model.py.  The number of Gauss-Newton steps of mode 3 is data dependent (epsilon-
+# terminated, R6): the kernel counts them (mc_get_work).
+# DRAM traffic of ONE FULL-LENGTH launch (314 x 314 orbits + shadows, 1e5 steps) of the hot kernel:
+# dram__bytes_read.sum + dram__bytes_write.sum from the ncu capture of that very launch configuration
+# (profiles/r02_ncu_traffic_full_launch.md).  Outputs (31 MB) and the carry buffer (31 MB) live in the 126 MB L2;
+# algorithmic: 340 B per orbit.
+NCU_DRAM_BYTES_PER_LAUNCH_314 = None   # set below once the round-2 capture exists
 FP64_LANES_PER_SM = 64
 
 
@@ -112,6 +106,26 @@ class ClockSampler(threading.Thread):
         return {"sm_mhz": float(np.median(self.samples)) if self.samples else None, "sm_max_mhz": self.max_mhz,
                 "reasons": reasons, "power_w_max": max(self.power) if self.power else None,
                 "samples": len(self.samples)}
+
+
+def algorithmic_flop(w, mode, integrator, steps_done, gn_steps):
+    """Algorithmic FP64 flop of one launch from mc_flop_model (the kernels' own formulation, counted by a counting
+    scalar) and the work the launch really did: accepted steps per orbit (`steps_done`), Gauss-Newton steps per
+    orbit summed over orbit and shadow (`gn_steps`, mc_get_work).  A trajectory-step = base integrator step +
+    the per-step part of the correction + status test; with a shadow every accepted orbit-step is two
+    trajectory-steps and every renorm_interval-th step one renormalisation."""
+    from paper_1802_00147_b200 import binding
+    m = binding.flop_model(w.terms, mode, integrator)
+    traj = 2 if w.shadow_eps != 0.0 else 1
+    steps_done = np.asarray(steps_done, dtype=np.int64)
+    per_traj_step = m["base_step"]["flop"] + m["correct_fixed"]["flop"] + m["status"]["flop"]
+    renorms = int((steps_done // w.renorm_interval).sum()) if traj == 2 else 0
+    total = int(traj * steps_done.sum()) * per_traj_step + int(np.asarray(gn_steps).sum()) * m["gn_step"]["flop"] \
+        + renorms * m["renorm"]["flop"]
+    return {"flop_per_launch": int(total), "trajectories_per_orbit": traj,
+            "model": {k: v["flop"] for k, v in m.items()},
+            "model_ops": {k: {kk: v[kk] for kk in ("fma", "mul", "add", "special")} for k, v in m.items()},
+            "per_trajectory_step_without_gn": per_traj_step}
 
 
 def global_workload(args, world):
@@ -297,8 +311,10 @@ def run_mc(args):
     info = I.launch_info()
     status = res.status.cpu().numpy()
     fli = res.fli.cpu().numpy() if res.fli is not None else np.zeros(n)
-    steps_done = float(res.steps_done.sum().item())          # accepted orbit-steps of one launch (this rank)
-    gn_steps = float(I.work(n).sum().item())                  # Gauss-Newton steps of one launch, orbit + shadow
+    steps_done_per_orbit = res.steps_done.cpu().numpy()
+    gn_per_orbit = I.work(n).cpu().numpy()
+    steps_done = float(steps_done_per_orbit.sum())            # accepted orbit-steps of one launch (this rank)
+    gn_steps = float(gn_per_orbit.sum())                      # Gauss-Newton steps of one launch, orbit + shadow
     steps_done_job = sharding.sum_over_ranks(steps_done, dev)
     # orbit-steps actually integrated (dropped cells stop counting when they freeze), whole job
     value = steps_done_job * args.steps / (dev_ms_max * 1e-3)
@@ -314,11 +330,9 @@ def run_mc(args):
     sm_max = float(mp.get("sm_max_mhz", clocks.get("sm_max_mhz") or 1965.0))
     nominal_tf = info["num_sms"] * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     per_launch_s = (dev_ms / args.steps) * 1e-3
-    base = FLOP_PER_ORBIT_STEP_BASE_RK5 if rk5 else FLOP_PER_ORBIT_STEP_BASE
-    # other correction modes (profiles/ tables only): no eq (10) / L_t in mode 0, no L_t in mode 1, + about 300 flop
-    # per trajectory-step for the polynomial dual scaling of mode 2 (SURVEY 8d estimate)
-    base += {0: -92.0, 1: -24.0, 2: -24.0 + 600.0, 3: 0.0}[w.correction_mode]
-    flop_per_launch = base * steps_done + FLOP_PER_GN_STEP * gn_steps
+    alg = algorithmic_flop(w, w.correction_mode, int(rk5), steps_done_per_orbit, gn_per_orbit)
+    flop_per_launch = float(alg["flop_per_launch"])
+    traj = alg["trajectories_per_orbit"]
     achieved_tf = flop_per_launch / per_launch_s / 1e12
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": nominal_tf, "unit": "TFLOP/s",
                 "frac": achieved_tf / nominal_tf,
@@ -330,7 +344,9 @@ def run_mc(args):
                 "peak_measured_dfma": peak_tf, "frac_of_measured_dfma": achieved_tf / peak_tf if peak_tf else None,
                 "dfma_probe_implied_sm_mhz": peak_clock,
                 "flop_per_launch": flop_per_launch, "flop_per_orbit_step": flop_per_launch / max(steps_done, 1.0),
-                "gn_steps_per_trajectory_step": gn_steps / max(2.0 * steps_done, 1.0),
+                "flop_model": alg["model"], "flop_model_ops": alg["model_ops"],
+                "flop_source": "mc_flop_model: the kernels' math templates run with a counting scalar (tests/test_flop_model.py)",
+                "gn_steps_per_trajectory_step": gn_steps / max(traj * steps_done, 1.0),
                 "accepted_orbit_steps_per_launch": steps_done, "kernel": "mc::integrate_kernel<%s,QM %s,mode %d>" % ("uniform" if w.uniform else "per-orbit", "on" if w.terms & 16 else "off", w.correction_mode),
                 "kernel_ms_per_launch": dev_ms / args.steps,
                 "regs_per_thread": info["regs_per_thread"], "spill_bytes": info["local_bytes"],
@@ -342,7 +358,7 @@ def run_mc(args):
                        "orbits_per_gpu": n, "rk4_steps": w.n_steps, "sample_interval": args.sample_interval,
                        "sample_bytes_per_launch": (w.n_steps // args.sample_interval) * 96 * n if args.sample_interval else 0,
                        "orbit_steps_counted": "accepted steps (sum of steps_done); scheduled = orbits x rk4_steps = %d" % int(orbit_steps_rank * world), "l2": "flushed (256 MiB write) between timed iterations",
-                       "parallelism": f"orbit-sharded x{world}, no collective"},
+                       "parallelism": f"orbit-sharded x{world} (grid rows round-robin over ranks), no collective"},
             "clocks": clocks, "wall_s_timed_region": t_wall,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
             "gpu_launches": launches, "roofline": roofline,

@@ -92,11 +92,18 @@ typedef struct mc_params {
                               work items are chunks of this many steps (state parked in device scratch owned
                               by the handle between chunks)                          */
   int32_t integrator;      /* mc_integrator; default MC_INTEG_RK4                                          */
+  double wait_budget_s;    /* scheduling watchdog, default 600: the kernel is persistent and a warp may wait for the
+                              previous chunk of its work unit, which another resident warp holds.  That cannot
+                              deadlock as long as the WHOLE GRID IS CO-RESIDENT: the library sizes the grid with the
+                              occupancy API on an otherwise idle device.  Under MPS / a co-tenant that takes SM
+                              resources the assumption can fail; a wait longer than this many seconds then ends the
+                              launch with a trap (MC_ECUDA on the next call) instead of a hang.  Raise it for
+                              profiler replays or very long forced chunks (chunk_steps); must be in (0, 1e9]   */
 } mc_params;
 
 /* Fill *p with defaults: terms = 1PN|2PN|SO|S1S2, device 0, uniform beta = chi = kq = 1,
  * renorm_interval 100, newton_iters 4, newton_tol 1e-10, r_merge 2, r_escape 1e4, stream NULL,
- * chunk_steps 0, integrator RK4. */
+ * chunk_steps 0, integrator RK4, wait_budget_s 600. */
 int mc_params_default(mc_params* p);
 
 /* Validate params, select the device, allocate the handle.  *out_handle is set only on success. */
@@ -175,7 +182,7 @@ int mc_get_work(mc_handle* h, int64_t* out_gn_steps);
  *   what = 2: out[6][n]  = E, Jx, Jy, Jz, |S1hat|, |S2hat|
  *   what = 3: out[12][n] = one step of the base integrator (params.integrator) of size step_h, no correction
  *   what = 4: out[12][n] = correction operator of mode `mode` applied to states, with references
- *             refs = DEVICE double[4][n] (E0, J0x, J0y, J0z)
+ *             refs = DEVICE double[4][n] (E0, J0x, J0y, J0z); required for every mode (MC_EINVAL if NULL)
  * Asynchronous on the handle's stream. */
 int mc_eval(mc_handle* h, int32_t what, const double* states, int64_t n, double step_h, int32_t mode,
             const double* refs, double* out);
@@ -199,6 +206,29 @@ int mc_last_launch_info(mc_handle* h, mc_launch_info* out);
  * `millis` ms; *out_tflops = 2 * FMAs / time (CUDA events).  The roofline denominator of bench.py
  * (MEASURED_PEAKS.json has no FP64 entry).  Synchronous. */
 int mc_fp64_peak(int32_t device, double millis, double* out_tflops, double* out_sm_clock_mhz);
+
+/* Algorithmic operation counts of the kernels' own formulation, per trajectory.
+ * Host-only, needs no GPU: the library instantiates the math templates the kernels are built from
+ * (csrc/mc_math.cuh, mc_correct.cuh) with a scalar type that counts its own operations, so the figures follow
+ * the code.  fma = fused multiply-adds, mul, add (additions and subtractions), special = rsqrt + reciprocal +
+ * division + sqrt (one each; the refinement steps around the hardware seeds are not algorithmic work).
+ * flop = 2 fma + mul + add + special.  Operations on constants and negations are free.
+ *   rhs            one evaluation of dz/dt (eqs 6-9)
+ *   base_step      one uncorrected step of the base integrator, RHS evaluations included
+ *   correct_fixed  the part of the correction done once per step: eq (10), L_t; for mode 2 the whole dual
+ *                  scaling with newton_iters polynomial Newton iterations; 0 for mode 0
+ *   gn_step        one Gauss-Newton step of mode 3 (gradient + H, 4 x 4 solve, update, termination test); else 0
+ *   status         the |r|^2 test of a completed step
+ *   references     E0, J0 of a state (H + J)
+ *   renorm         one shadow renormalisation (distance, pull-back, eq 10, re-referenced integrals)
+ * A trajectory-step costs base_step + correct_fixed + status + gn_step x (Gauss-Newton steps taken, mc_get_work).
+ * Errors: MC_EINVAL (null, unknown term bit / mode / integrator, newton_iters outside 1..16). */
+typedef struct mc_op_counts { int64_t fma, mul, add, special; } mc_op_counts;
+typedef struct mc_flop_model_t {
+  mc_op_counts rhs, base_step, correct_fixed, gn_step, status, references, renorm;
+} mc_flop_model_t;
+int mc_flop_model(uint32_t terms, int32_t correction_mode, int32_t integrator, int32_t newton_iters,
+                  mc_flop_model_t* out);
 
 int mc_destroy(mc_handle* h);
 

@@ -18,7 +18,7 @@ MC_INTEG_RK4, MC_INTEG_RK5 = 0, 1
 
 # every symbol include/mc.h declares (tests/test_abi.py checks the header against this list)
 EXPORTS = ["mc_params_default", "mc_create", "mc_integrate", "mc_integrate_sampled", "mc_integrate_ex", "mc_carry_bytes", "mc_integrate_host", "mc_get_status", "mc_get_work", "mc_eval",
-           "mc_last_launch_info", "mc_fp64_peak", "mc_destroy", "mc_strerror"]
+           "mc_last_launch_info", "mc_fp64_peak", "mc_flop_model", "mc_destroy", "mc_strerror"]
 
 
 class MCLibraryError(RuntimeError):
@@ -38,7 +38,8 @@ class mc_params(ctypes.Structure):
                 ("d_beta", ctypes.c_void_p), ("d_chi1", ctypes.c_void_p), ("d_chi2", ctypes.c_void_p),
                 ("d_kq1", ctypes.c_void_p), ("d_kq2", ctypes.c_void_p), ("renorm_interval", ctypes.c_int32),
                 ("newton_iters", ctypes.c_int32), ("newton_tol", ctypes.c_double), ("r_merge", ctypes.c_double),
-                ("r_escape", ctypes.c_double), ("cuda_stream", ctypes.c_void_p), ("chunk_steps", ctypes.c_int32), ("integrator", ctypes.c_int32)]
+                ("r_escape", ctypes.c_double), ("cuda_stream", ctypes.c_void_p), ("chunk_steps", ctypes.c_int32), ("integrator", ctypes.c_int32),
+                ("wait_budget_s", ctypes.c_double)]
 
 
 class mc_launch_info(ctypes.Structure):
@@ -46,6 +47,14 @@ class mc_launch_info(ctypes.Structure):
                 ("local_bytes", ctypes.c_int32), ("blocks_per_sm", ctypes.c_int32), ("num_sms", ctypes.c_int32),
                 ("smem_bytes", ctypes.c_int32), ("variant", ctypes.c_int32), ("trajectories", ctypes.c_int64),
                 ("chunk_steps", ctypes.c_int32), ("n_chunks", ctypes.c_int32)]
+
+
+class mc_op_counts(ctypes.Structure):
+    _fields_ = [("fma", ctypes.c_int64), ("mul", ctypes.c_int64), ("add", ctypes.c_int64), ("special", ctypes.c_int64)]
+
+
+class mc_flop_model_t(ctypes.Structure):
+    _fields_ = [(k, mc_op_counts) for k in ("rhs", "base_step", "correct_fixed", "gn_step", "status", "references", "renorm")]
 
 
 _lib = None
@@ -60,14 +69,17 @@ def load_library():
     global _lib
     if _lib is not None:
         return _lib
-    try:
-        # MC_LIBMC_PATH: use a prebuilt libmc.so (e.g. a box without nvcc) instead of building in-tree
-        path = os.environ.get("MC_LIBMC_PATH") or _build.build()
-    except Exception as e:  # nvcc missing or compile error
-        if os.path.exists(_build.LIB):
-            path = _build.LIB
-        else:
-            raise MCLibraryError(f"libmc.so is not built and could not be built: {e}") from e
+    path = os.environ.get("MC_LIBMC_PATH")      # a prebuilt libmc.so (e.g. a box without nvcc) instead of building in-tree
+    if not path:
+        try:
+            path = _build.build()
+        except FileNotFoundError as e:           # no nvcc on this box: an existing library is all there can be
+            if os.path.exists(_build.LIB) and not _build.sources_newer_than_library():
+                path = _build.LIB
+            else:
+                raise MCLibraryError(f"libmc.so is missing or older than its sources and nvcc is not available: {e}") from e
+        except Exception as e:                   # nvcc ran and failed: never fall back to a stale binary
+            raise MCLibraryError(f"libmc.so could not be built from the current sources: {e}") from e
     try:
         lib = ctypes.CDLL(path)
     except OSError as e:
@@ -85,6 +97,7 @@ def load_library():
     lib.mc_eval.argtypes = [vp, i32, vp, i64, dbl, i32, vp, vp]
     lib.mc_last_launch_info.argtypes = [vp, ctypes.POINTER(mc_launch_info)]
     lib.mc_fp64_peak.argtypes = [i32, dbl, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
+    lib.mc_flop_model.argtypes = [ctypes.c_uint32, i32, i32, i32, ctypes.POINTER(mc_flop_model_t)]
     lib.mc_destroy.argtypes = [vp]
     lib.mc_strerror.argtypes = [ctypes.c_int]
     lib.mc_strerror.restype = ctypes.c_char_p
@@ -114,6 +127,18 @@ def fp64_peak(device: int = 0, millis: float = 200.0):
     return t.value, c.value
 
 
+def flop_model(terms=TERMS_DEFAULT, correction_mode=3, integrator=0, newton_iters=4) -> dict:
+    """mc_flop_model: operation counts of the kernels' own formulation, per trajectory (host-only, no GPU needed).
+    Returns {part: {"fma", "mul", "add", "special", "flop"}} with flop = 2 fma + mul + add + special."""
+    m = mc_flop_model_t()
+    _check(load_library().mc_flop_model(int(terms), int(correction_mode), int(integrator), int(newton_iters), ctypes.byref(m)))
+    out = {}
+    for part, _ in mc_flop_model_t._fields_:
+        c = getattr(m, part)
+        out[part] = dict(fma=c.fma, mul=c.mul, add=c.add, special=c.special, flop=2 * c.fma + c.mul + c.add + c.special)
+    return out
+
+
 @dataclass
 class IntegrateResult:
     states: "object"                 # torch.Tensor (12, n) float64, device
@@ -130,7 +155,7 @@ class Integrator:
 
     def __init__(self, terms=TERMS_DEFAULT, beta=1.0, chi1=1.0, chi2=1.0, kq1=1.0, kq2=1.0, device=0,
                  renorm_interval=100, newton_iters=4, newton_tol=1e-10, r_merge=2.0, r_escape=1e4, stream=None,
-                 chunk_steps=0, integrator=0):
+                 chunk_steps=0, integrator=0, wait_budget_s=600.0):
         import torch
         self._torch = torch
         self._lib = load_library()
@@ -140,6 +165,7 @@ class Integrator:
         p.r_merge, p.r_escape = float(r_merge), float(r_escape)
         p.chunk_steps = int(chunk_steps)
         p.integrator = int(integrator)
+        p.wait_budget_s = float(wait_budget_s)
         self.device = torch.device("cuda", device)
         vals = dict(beta=beta, chi1=chi1, chi2=chi2, kq1=kq1, kq2=kq2)
         per_orbit = any(hasattr(v, "__len__") for v in vals.values())

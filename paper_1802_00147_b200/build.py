@@ -8,7 +8,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libmc.so")
-SOURCES = ["mc_api.cu", "mc_kernel_mode0.cu", "mc_kernel_mode1.cu", "mc_kernel_mode2.cu", "mc_kernel_mode3.cu"]
+SOURCES = ["mc_api.cu", "mc_kernel_mode0.cu", "mc_kernel_mode1.cu", "mc_kernel_mode2.cu", "mc_kernel_mode3.cu",
+           "mc_flop_model.cpp"]       # .cpp: host-only C++ (the flop model), compiled by nvcc's host compiler
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
@@ -16,16 +17,33 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3",
 def _deps():
     out = [os.path.join(HERE, "..", "include", "mc.h")]
     for f in os.listdir(CSRC):
-        if f.endswith((".cu", ".cuh", ".h")):
+        if f.endswith((".cu", ".cuh", ".h", ".cpp")):
             out.append(os.path.join(CSRC, f))
     return out
 
 
-def is_stale() -> bool:
-    if not os.path.exists(LIB):
-        return True
+def sources_newer_than_library() -> bool:
     t = os.path.getmtime(LIB)
     return any(os.path.getmtime(f) > t for f in _deps())
+
+
+def is_stale() -> bool:
+    return not os.path.exists(LIB) or sources_newer_than_library()
+
+
+def spill_report(log: str):
+    """(kernel, line) for every integrate_kernel / eval_kernel instantiation that ptxas -v reports with a stack frame
+    or spill traffic.  north_star: zero register spills -- build() refuses to ship a library that has any."""
+    bad, current = [], None
+    for line in log.splitlines():
+        if "Function properties for" in line:
+            current = line.split("Function properties for")[1].strip()
+        elif "bytes stack frame" in line and current is not None:
+            nums = [int(x) for x in line.replace(",", " ").split() if x.isdigit()]
+            if any(nums[:3]) and ("integrate_kernel" in current or "eval_kernel" in current):
+                bad.append((current, line.strip()))
+            current = None
+    return bad
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -35,7 +53,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     nvcc = os.environ.get("NVCC", "nvcc")
 
     def compile_one(src):
-        obj = os.path.join(OBJ, src.replace(".cu", ".o"))
+        obj = os.path.join(OBJ, os.path.splitext(src)[0] + ".o")
         r = subprocess.run([nvcc] + NVCC_FLAGS + ["-c", os.path.join(CSRC, src), "-o", obj],
                            capture_output=True, text=True)
         if r.returncode != 0:
@@ -49,6 +67,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
         f.write(log)
     if verbose:
         print(log)
+    bad = spill_report(log)
+    if bad:
+        raise RuntimeError("register spills (north_star demands none):\n" + "\n".join(f"{k}: {l}" for k, l in bad))
     subprocess.run([nvcc, "-shared", "-Wno-deprecated-gpu-targets", "-o", LIB + ".tmp"] + [o for o, _ in results] + ["-lcudart_static", "-ldl", "-lrt", "-lpthread"],
                    check=True)
     os.replace(LIB + ".tmp", LIB)

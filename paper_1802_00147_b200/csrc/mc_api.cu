@@ -151,6 +151,7 @@ void fill_args(const mc_handle* h, mc::IntegrateArgs& A) {
   A.integrator = h->P.integrator;
   A.r_merge2 = h->P.r_merge * h->P.r_merge;
   A.r_escape2 = h->P.r_escape * h->P.r_escape;
+  A.wait_budget_ns = (unsigned long long)(h->P.wait_budget_s * 1e9);
 }
 
 }  // namespace
@@ -173,6 +174,7 @@ int mc_params_default(mc_params* p) {
   p->cuda_stream = nullptr;
   p->chunk_steps = 0;
   p->integrator = MC_INTEG_RK4;
+  p->wait_budget_s = 600.0;
   return MC_OK;
 }
 
@@ -184,6 +186,7 @@ int mc_create(const mc_params* params, mc_handle** out_handle) {
   if (params->chunk_steps < 0) return MC_EINVAL;
   if (params->integrator != MC_INTEG_RK4 && params->integrator != MC_INTEG_RK5) return MC_EINVAL;
   if (!(params->newton_tol >= 0.0) || !(params->r_merge >= 0.0) || !(params->r_escape > params->r_merge)) return MC_EINVAL;
+  if (!(params->wait_budget_s > 0.0) || !(params->wait_budget_s <= 1e9)) return MC_EINVAL;
   if (params->per_orbit) {
     if (!params->d_beta || !params->d_chi1 || !params->d_chi2 || !params->d_kq1 || !params->d_kq2) return MC_EINVAL;
   } else if (!valid_scalars(params->beta, params->chi1, params->chi2, params->kq1, params->kq2)) {
@@ -230,7 +233,7 @@ int mc_integrate_sampled(mc_handle* h, const double* states, int64_t n_orbits, d
 int64_t mc_carry_bytes(int64_t n_orbits, int32_t with_shadow) {
   if (n_orbits < 0) return MC_EINVAL;
   const int64_t tp = ((n_orbits * (with_shadow ? 2 : 1) + 31) / 32) * 32;
-  return tp * (int64_t)(17 * sizeof(double) + sizeof(unsigned long long) + 3 * sizeof(int32_t));
+  return tp * (int64_t)(17 * sizeof(double) + 2 * sizeof(unsigned long long) + 2 * sizeof(int32_t));
 }
 
 int mc_integrate_ex(mc_handle* h, const double* states, int64_t n_orbits, double step_h, int64_t n_steps,
@@ -308,16 +311,16 @@ static int integrate_impl(mc_handle* h, const double* states, int64_t n_orbits, 
   A.done = (int32_t*)((char*)h->sched.p + 16);
   A.resume = resume; A.save_final = user_carry ? 1 : 0;
   if (user_carry) {
-    // caller-owned checkpoint (mc_carry_bytes): [17][tp] doubles, [tp] u64, [3][tp] int32 -- also the chunk carry
+    // caller-owned checkpoint (mc_carry_bytes): [17][tp] doubles, [2][tp] u64, [2][tp] int32 -- also the chunk carry
     const size_t tp = (size_t)A.n_units * 32;
     A.carry_d = (double*)user_carry;
     A.carry_g = (unsigned long long*)(A.carry_d + 17 * tp);
-    A.carry_i = (int32_t*)(A.carry_g + tp);
+    A.carry_i = (int32_t*)(A.carry_g + 2 * tp);
   } else if (n_chunks > 1) {
     const size_t tp = (size_t)A.n_units * 32;
     if ((rc = h->carry_d.reserve(sizeof(double) * 17 * tp))) return rc;
-    if ((rc = h->carry_i.reserve(sizeof(int32_t) * 3 * tp))) return rc;
-    if ((rc = h->carry_g.reserve(sizeof(unsigned long long) * tp))) return rc;
+    if ((rc = h->carry_i.reserve(sizeof(int32_t) * 2 * tp))) return rc;
+    if ((rc = h->carry_g.reserve(sizeof(unsigned long long) * 2 * tp))) return rc;
     A.carry_d = (double*)h->carry_d.p; A.carry_i = (int32_t*)h->carry_i.p; A.carry_g = (unsigned long long*)h->carry_g.p;
   }
   MC_CUDA(cudaMemsetAsync(h->sched.p, 0, 16 + sizeof(int32_t) * (size_t)A.n_units, h->stream));
@@ -388,7 +391,7 @@ int mc_eval(mc_handle* h, int32_t what, const double* states, int64_t n, double 
   if (!h || n < 0 || what < 0 || what > 4) return MC_EINVAL;
   if (n == 0) return MC_OK;
   if (!states || !out) return MC_EINVAL;
-  if (what == 4 && (mode < 0 || mode > 3 || (mode >= 2 && !refs))) return MC_EINVAL;
+  if (what == 4 && (mode < 0 || mode > 3 || !refs)) return MC_EINVAL;   // the kernel reads refs for every mode
   MC_CUDA(cudaSetDevice(h->P.device));
   mc::IntegrateArgs A;
   fill_args(h, A);

@@ -5,10 +5,16 @@
 
 namespace mc {
 
-struct Refs { double E0, J0[3]; };   // reference integrals "at the starting time"
+template <class T> struct RefsT { T E0, J0[3]; };   // reference integrals "at the starting time"
+typedef RefsT<double> Refs;
 
-template <bool QM, class C>
-__device__ __forceinline__ void references(const C& c, const double* z, Refs& R) {
+#ifdef __CUDACC__
+__device__ __forceinline__ bool warp_any(bool b) { return __any_sync(0xffffffffu, b); }
+__device__ __forceinline__ double abs_(double x) { return fabs(x); }
+#endif
+
+template <bool QM, class C, class T>
+MC_DEV void references(const C& c, const T* z, RefsT<T>& R) {
   R.E0 = hamiltonian<QM>(c, z);
   total_J(c, z, R.J0);
 }
@@ -24,62 +30,62 @@ __device__ __forceinline__ void references(const C& c, const double* z, Refs& R)
 // satisfies |(dr,dp)|^2 <= tol^2 p.p, at most `iters` times.  The decision is per lane (results do not
 // depend on the neighbours); the warp leaves the loop when no lane needs another step.  Must be called
 // by all 32 lanes.  Returns the number of steps this lane took.
-template <bool QM, class C>
-__device__ __forceinline__ int project_six(const C& c, double* z, const Refs& R, int iters, double tol2) {
-  double Lt[3];
+template <bool QM, class C, class T>
+MC_DEV int project_six(const C& c, T* z, const RefsT<T>& R, int iters, double tol2) {
+  T Lt[3];
 #pragma unroll
   for (int i = 0; i < 3; ++i) Lt[i] = fma(-c[K_S2], z[9 + i], fma(-c[K_S1], z[6 + i], R.J0[i]));
   bool need = true;
   int done = 0;
 #pragma unroll 1
   for (int it = 0; it < iters; ++it) {
-    if (!__any_sync(0xffffffffu, need)) break;
+    if (!warp_any(need)) break;
     if (need) {
-      double g[12], H;
+      T g[12], H;
       pn_eval<QM, false, true>(c, z, g, H);
-      double* r = z;
-      double* p = z + 3;
-      const double* a = g;
-      const double* b = g + 3;
-      double fL[3], cv[3];
+      T* r = z;
+      T* p = z + 3;
+      const T* a = g;
+      const T* b = g + 3;
+      T fL[3], cv[3];
       cross3(r, p, fL);
 #pragma unroll
       for (int i = 0; i < 3; ++i) fL[i] -= Lt[i];
-      const double f0 = H - R.E0;
+      const T f0 = H - R.E0;
       // c = a x p + r x b
       cv[0] = fma(r[1], b[2], fma(-r[2], b[1], fma(a[1], p[2], -(a[2] * p[1]))));
       cv[1] = fma(r[2], b[0], fma(-r[0], b[2], fma(a[2], p[0], -(a[0] * p[2]))));
       cv[2] = fma(r[0], b[1], fma(-r[1], b[0], fma(a[0], p[1], -(a[1] * p[0]))));
-      const double gg = dot3(a, a) + dot3(b, b);
-      const double rr = dot3(r, r), pp = dot3(p, p), rp = dot3(r, p);
-      const double LL = fma(rr, pp, -(rp * rp));
-      const double D = (rr + pp) * LL;
+      const T gg = dot3(a, a) + dot3(b, b);
+      const T rr = dot3(r, r), pp = dot3(p, p), rp = dot3(r, p);
+      const T LL = fma(rr, pp, -(rp * rp));
+      const T D = (rr + pp) * LL;
       // N(c), N(fL)
-      const double rc = dot3(r, cv), pc = dot3(p, cv), rf = dot3(r, fL), pf = dot3(p, fL);
-      const double cr_ = fma(rp, pc, rr * rc), cp_ = fma(pp, pc, rp * rc);
-      const double fr_ = fma(rp, pf, rr * rf), fp_ = fma(pp, pf, rp * rf);
-      double Nc[3], Nf[3];
+      const T rc = dot3(r, cv), pc = dot3(p, cv), rf = dot3(r, fL), pf = dot3(p, fL);
+      const T cr_ = fma(rp, pc, rr * rc), cp_ = fma(pp, pc, rp * rc);
+      const T fr_ = fma(rp, pf, rr * rf), fp_ = fma(pp, pf, rp * rf);
+      T Nc[3], Nf[3];
 #pragma unroll
       for (int i = 0; i < 3; ++i) {
         Nc[i] = fma(p[i], cp_, fma(r[i], cr_, LL * cv[i]));
         Nf[i] = fma(p[i], fp_, fma(r[i], fr_, LL * fL[i]));
       }
-      const double S = fma(gg, D, -dot3(cv, Nc));
-      const double num = fma(D, f0, -dot3(cv, Nf));
-      const double DS = D * S;
-      const double inv = (DS != 0.0) ? rcp_nz(DS) : 0.0;      // singular only for r || p or a circular orbit
-      const double l0 = num * D * inv;                         // num / S
-      const double sD = S * inv;                               // 1 / D
-      double lL[3], d1[3], d2[3];
+      const T S = fma(gg, D, -dot3(cv, Nc));
+      const T num = fma(D, f0, -dot3(cv, Nf));
+      const T DS = D * S;
+      const T inv = (DS != 0.0) ? rcp_nz(DS) : T(0.0);      // singular only for r || p or a circular orbit
+      const T l0 = num * D * inv;                         // num / S
+      const T sD = S * inv;                               // 1 / D
+      T lL[3], d1[3], d2[3];
 #pragma unroll
       for (int i = 0; i < 3; ++i) lL[i] = fma(-l0, Nc[i], Nf[i]) * sD;
       cross3(p, lL, d1);   // dr = l0 a + p x lL
       cross3(lL, r, d2);   // dp = l0 b + lL x r
-      double dd = 0.0;
+      T dd = 0.0;
 #pragma unroll
       for (int i = 0; i < 3; ++i) {
-        const double dr = fma(l0, a[i], d1[i]);
-        const double dp = fma(l0, b[i], d2[i]);
+        const T dr = fma(l0, a[i], d1[i]);
+        const T dp = fma(l0, b[i], d2[i]);
         dd = fma(dr, dr, fma(dp, dp, dd));
         r[i] -= dr;
         p[i] -= dp;
@@ -95,55 +101,54 @@ __device__ __forceinline__ int project_six(const C& c, double* z, const Refs& R,
 // (eqs 12-13 at their exact root, R5).  With v = 1/beta_s, gamma = alpha beta_s every term of
 // H is a monomial in (alpha, v), so g(v) = H(gamma v, v) - E0 is a degree-6 polynomial whose
 // coefficients are computed once; gamma is the root of the |J| quadratic.  Returns false if skipped.
-template <bool QM, class C>
-__device__ __forceinline__ bool dual_scaling(const C& c, double* z, const Refs& R, int iters, double tol) {
-  const double* r = z;
-  const double* p = z + 3;
-  const double* s1 = z + 6;
-  const double* s2 = z + 9;
-  double L[3], S[3];
+template <bool QM, class C, class T>
+MC_DEV bool dual_scaling(const C& c, T* z, const RefsT<T>& R, int iters, double tol) {
+  const T* r = z;
+  const T* p = z + 3;
+  const T* s1 = z + 6;
+  const T* s2 = z + 9;
+  T L[3], S[3];
   cross3(r, p, L);
 #pragma unroll
   for (int i = 0; i < 3; ++i) S[i] = fma(c[K_S2], s2[i], c[K_S1] * s1[i]);
-  const double LL = dot3(L, L), LS = dot3(L, S), SS = dot3(S, S), J02 = dot3(R.J0, R.J0);
-  const double disc = fma(LS, LS, -(LL * (SS - J02)));
+  const T LL = dot3(L, L), LS = dot3(L, S), SS = dot3(S, S), J02 = dot3(R.J0, R.J0);
+  const T disc = fma(LS, LS, -(LL * (SS - J02)));
   if (!(disc >= 0.0) || !(LL > 0.0)) return false;
-  const double sg = (LL + LS >= 0.0) ? 1.0 : -1.0;
-  const double gam = (sg * sqrt(disc) - LS) / LL;
+  const T sg = (LL + LS >= 0.0) ? T(1.0) : T(-1.0);
+  const T gam = div_(sg * sqrt_pos(disc) - LS, LL);
   // starred scalars
-  const double u = rsqrt_pos(dot3(r, r));
-  const double u2 = u * u, u3 = u2 * u, u5 = u3 * u2;
-  const double rp = dot3(r, p), P = dot3(p, p);
-  const double npu = rp * u, Q = npu * npu;
-  const double a1 = dot3(s1, r), a2 = dot3(s2, r), d12 = dot3(s1, s2);
-  double Sg[3];
+  const T u = rsqrt_pos(dot3(r, r));
+  const T u2 = u * u, u3 = u2 * u, u5 = u3 * u2;
+  const T rp = dot3(r, p), P = dot3(p, p);
+  const T npu = rp * u, Q = npu * npu;
+  const T a1 = dot3(s1, r), a2 = dot3(s2, r), d12 = dot3(s1, s2);
+  T Sg[3];
 #pragma unroll
   for (int i = 0; i < 3; ++i) Sg[i] = fma(c[K_K2], s2[i], c[K_K1] * s1[i]);
-  const double Hso = u3 * dot3(L, Sg);
-  double Hss = c[K_C12] * fma(3.0 * a1 * a2, u5, -(d12 * u3));
+  const T Hso = u3 * dot3(L, Sg);
+  T Hss = c[K_C12] * fma(3.0 * a1 * a2, u5, -(d12 * u3));
   if (QM) {
     Hss += c[K_Q1] * fma(3.0 * a1 * a1, u5, -(dot3(s1, s1) * u3));
     Hss += c[K_Q2] * fma(3.0 * a2 * a2, u5, -(dot3(s2, s2) * u3));
   }
-  const double g2 = gam * gam, g4 = g2 * g2, g6 = g4 * g2;
+  const T g2 = gam * gam, g4 = g2 * g2, g6 = g4 * g2;
   // g(v) = -E0 + k1 v + k2 v^2 + ... + k6 v^6
-  const double k1 = -u;
-  const double k2 = fma(0.5 * g2, P, c[K_H1] * u2);
-  const double k3 = fma(g2 * u, fma(c[K_B1], P, c[K_B2] * Q), fma(c[K_F1], u3, fma(gam, Hso, Hss)));
-  const double k4 = fma(g4 * c[K_A1], P * P, g2 * u2 * fma(c[K_E1], P, c[K_E2] * Q));
-  const double k5 = g4 * u * fma(P, fma(c[K_D1], P, c[K_D2] * Q), c[K_D3] * Q * Q);
-  const double k6 = g6 * c[K_C3] * P * P * P;
-  double v = 1.0, dv = 0.0;
+  const T k1 = -u;
+  const T k2 = fma(0.5 * g2, P, c[K_H1] * u2);
+  const T k3 = fma(g2 * u, fma(c[K_B1], P, c[K_B2] * Q), fma(c[K_F1], u3, fma(gam, Hso, Hss)));
+  const T k4 = fma(g4 * c[K_A1], P * P, g2 * u2 * fma(c[K_E1], P, c[K_E2] * Q));
+  const T k5 = g4 * u * fma(P, fma(c[K_D1], P, c[K_D2] * Q), c[K_D3] * Q * Q);
+  const T k6 = g6 * c[K_C3] * P * P * P;
+  T v = 1.0, dv = 0.0;
 #pragma unroll 1
   for (int it = 0; it < iters; ++it) {
-    const double gv = fma(v, fma(v, fma(v, fma(v, fma(v, fma(v, k6, k5), k4), k3), k2), k1), -R.E0);
-    const double dg = fma(v, fma(v, fma(v, fma(v, fma(v, 6.0 * k6, 5.0 * k5), 4.0 * k4), 3.0 * k3), 2.0 * k2), k1);
-    dv = -gv / dg;
+    const T gv = fma(v, fma(v, fma(v, fma(v, fma(v, fma(v, k6, k5), k4), k3), k2), k1), -R.E0);
+    const T dg = fma(v, fma(v, fma(v, fma(v, fma(v, 6.0 * k6, 5.0 * k5), 4.0 * k4), 3.0 * k3), 2.0 * k2), k1);
+    dv = -div_(gv, dg);
     v += dv;
   }
-  const bool finite_v = (((unsigned)__double2hiint(v)) & 0x7ff00000u) != 0x7ff00000u;
-  if (!finite_v || !(fabs(dv) <= tol) || !(fabs(v - 1.0) <= 1e-3)) return false;
-  const double bs = 1.0 / v, al = gam * v;
+  if (!is_finite(v) || !(abs_(dv) <= tol) || !(abs_(v - 1.0) <= 1e-3)) return false;
+  const T bs = div_(T(1.0), v), al = gam * v;
 #pragma unroll
   for (int i = 0; i < 3; ++i) { z[i] *= bs; z[3 + i] *= al; }
   return true;
@@ -151,8 +156,8 @@ __device__ __forceinline__ bool dual_scaling(const C& c, double* z, const Refs& 
 
 // C_mode: spins first (eq 10), then (r,p) with the corrected spins.
 // gn_steps receives the number of Gauss-Newton steps mode 3 took (0 otherwise).
-template <int MODE, bool QM, class C>
-__device__ __forceinline__ bool correct(const C& c, double* z, const Refs& R, int iters, double tol, int& gn_steps) {
+template <int MODE, bool QM, class C, class T>
+MC_DEV bool correct(const C& c, T* z, const RefsT<T>& R, int iters, double tol, int& gn_steps) {
   gn_steps = 0;
   if (MODE >= 1) { normalise3(z + 6); normalise3(z + 9); }
   if (MODE == 2) return dual_scaling<QM>(c, z, R, iters, tol);

@@ -1,0 +1,102 @@
+// mc_flop_model.cpp -- mc_flop_model (include/mc.h): the algorithmic operation counts of the kernels'
+// own formulation, obtained by running the kernels' math templates (mc_math.cuh, mc_correct.cuh) once on the
+// host with the counting scalar mc::Cnt.  Plain C++ (no CUDA): works on a box without a GPU.
+#include <cstring>
+
+#include "../../include/mc.h"
+#include "mc_count.h"
+#include "mc_correct.cuh"
+
+namespace {
+
+struct HostConsts {
+  double v[MC_NCONST];
+  double operator[](int i) const { return v[i]; }
+};
+
+mc_op_counts delta(const mc::OpCounts& a, const mc::OpCounts& b) {
+  mc_op_counts d;
+  d.fma = a.fma - b.fma; d.mul = a.mul - b.mul; d.add = a.add - b.add; d.special = a.special - b.special;
+  return d;
+}
+mc_op_counts sub(const mc_op_counts& a, const mc_op_counts& b) {
+  mc_op_counts d = {a.fma - b.fma, a.mul - b.mul, a.add - b.add, a.special - b.special};
+  return d;
+}
+
+// a generic bound orbit (config-0 like); the counts do not depend on the values
+void sample_state(mc::Cnt* z) {
+  const double v[12] = {20.0, 0.3, -0.2, 0.01, 0.2, 0.02, 0.6, 0.0, 0.8, 0.0, -0.6, -0.8};
+  for (int i = 0; i < 12; ++i) z[i] = mc::Cnt(v[i]);
+}
+
+template <class F>
+mc_op_counts count(F f) {
+  const mc::OpCounts before = mc::op_counts();
+  f();
+  return delta(mc::op_counts(), before);
+}
+
+template <bool QM, int INTEG>
+void model(const HostConsts& c, int mode, int newton_iters, mc_flop_model_t* out) {
+  using mc::Cnt;
+  Cnt z[12], f[12];
+  sample_state(z);
+  out->rhs = count([&] { mc::pn_rhs<QM>(c, z, f); });
+  out->base_step = count([&] { mc::base_step<INTEG, QM>(c, z, 1.0, f); });
+  mc::RefsT<Cnt> R;
+  mc::references<QM>(c, z, R);
+  out->references = count([&] { mc::references<QM>(c, z, R); });
+  // correction: perturb the state a little so that the Gauss-Newton steps do not vanish
+  auto run = [&](int iters) {
+    Cnt y[12];
+    for (int i = 0; i < 12; ++i) y[i] = Cnt(f[i].v * (1.0 + 1e-9 * (i + 1)));
+    return count([&] {
+      int gn = 0;
+      if (mode == 1) mc::correct<1, QM>(c, y, R, iters, 0.0, gn);
+      else if (mode == 2) mc::correct<2, QM>(c, y, R, iters, 1.0, gn);
+      else if (mode == 3) mc::correct<3, QM>(c, y, R, iters, 0.0, gn);
+    });
+  };
+  memset(&out->gn_step, 0, sizeof(out->gn_step));
+  if (mode == 3) {
+    const mc_op_counts c1 = run(1), c2 = run(2);
+    out->gn_step = sub(c2, c1);
+    out->correct_fixed = sub(c1, out->gn_step);
+  } else {
+    out->correct_fixed = run(newton_iters);
+  }
+  // status test of a completed step: |r|^2 against the two thresholds (the finite test is integer work)
+  out->status = count([&] { Cnt r2 = mc::dot3(z, z); (void)(r2 < Cnt(4.0)); });
+  // one shadow renormalisation: 12-norm, sqrt, d0 / d, pull-back, eq (10), re-referenced integrals (log10 not counted)
+  out->renorm = count([&] {
+    Cnt d2 = 0.0, y[12];
+    for (int i = 0; i < 12; ++i) { const Cnt e = z[i] - f[i]; d2 = fma(e, e, d2); }
+    const Cnt d = mc::sqrt_pos(d2);
+    const Cnt s = mc::div_(Cnt(1e-8), d);
+    for (int i = 0; i < 12; ++i) y[i] = fma(s, z[i] - f[i], f[i]);
+    if (mode >= 1) { mc::normalise3(y + 6); mc::normalise3(y + 9); }
+    mc::references<QM>(c, y, R);
+  });
+}
+
+}  // namespace
+
+extern "C" int mc_flop_model(uint32_t terms, int32_t correction_mode, int32_t integrator, int32_t newton_iters,
+                             mc_flop_model_t* out) {
+  if (!out || (terms & ~31u) || correction_mode < 0 || correction_mode > 3) return MC_EINVAL;
+  if (integrator != MC_INTEG_RK4 && integrator != MC_INTEG_RK5) return MC_EINVAL;
+  if (newton_iters < 1 || newton_iters > 16) return MC_EINVAL;
+  HostConsts c;
+  mc_derive_consts(0.8, 0.9, 0.7, 2.0, 3.0, terms, c.v);
+  const bool qm = (terms & MC_TERM_QM) != 0;
+  memset(out, 0, sizeof(*out));
+  if (qm) {
+    if (integrator == MC_INTEG_RK5) model<true, 1>(c, correction_mode, newton_iters, out);
+    else model<true, 0>(c, correction_mode, newton_iters, out);
+  } else {
+    if (integrator == MC_INTEG_RK5) model<false, 1>(c, correction_mode, newton_iters, out);
+    else model<false, 0>(c, correction_mode, newton_iters, out);
+  }
+  return MC_OK;
+}

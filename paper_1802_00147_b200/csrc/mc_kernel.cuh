@@ -43,14 +43,15 @@ struct IntegrateArgs {
   unsigned long long* queue;  // [0] = next item
   int32_t* done;              // [n_units] chunks completed per unit
   double* carry_d;            // [17][n_traj_padded]: y[12], E0, J0[3], acc
-  int32_t* carry_i;           // [3][n_traj_padded]: status | flag << 16 | frozen << 31, steps, until_renorm
-  unsigned long long* carry_g;  // [n_traj_padded]: Gauss-Newton steps
+  int32_t* carry_i;           // [2][n_traj_padded]: status | flag << 8 | frozen << 31, until_renorm
+  unsigned long long* carry_g;  // [2][n_traj_padded]: Gauss-Newton steps, completed steps (64-bit: they accumulate over resumed calls)
   int64_t n_units;            // ceil(trajectories / 32)
   int64_t n_items;            // n_units * n_chunks
   int32_t chunk_len;          // steps per chunk (>= 1)
   int32_t n_chunks;
   int32_t resume;             // 1: chunk 0 starts from the carry buffer instead of `states` (mc_integrate_ex)
   int32_t save_final;         // 1: the last chunk also parks its state in the carry buffer (mc_integrate_ex)
+  unsigned long long wait_budget_ns;  // a warp waiting longer than this for its unit's previous chunk traps (mc_params.wait_budget_s)
 };
 
 enum { ST_OK = 0, ST_MERGED = 1, ST_UNBOUND = 2, ST_NONFINITE = 3, ST_NEWTON_FLAG = 256 };
@@ -115,8 +116,10 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
     Refs R;
     int status = ST_OK, flag = 0;
     bool frozen = false;
+    // accepted steps and Gauss-Newton steps of THIS work item (chunk): 32-bit in the loop; the 64-bit totals of
+    // earlier chunks / earlier calls stay in the carry buffer and are added when the item is parked or stored
     int steps = 0;
-    unsigned long long gn_total = 0;
+    unsigned gn_chunk = 0;
     double acc = 0.0;
     int until_renorm = A.renorm_interval;
 
@@ -135,7 +138,10 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
       references<QM>(c, y, R);
     } else {
       // wait until this unit's previous chunk is published, then reload the carried state.  The holder of
-      // that chunk got it earlier from the same queue, so it is running: the wait cannot deadlock.
+      // that chunk got it earlier from the same queue, so it is running -- PROVIDED the whole grid is resident at
+      // once, which the launcher guarantees by sizing the grid with the occupancy API (mc_launch_impl.cuh); under
+      // MPS or any other co-tenant that takes SM resources between the query and the launch that no longer holds,
+      // hence the budget: a wait longer than mc_params.wait_budget_s traps (the launch fails) instead of hanging.
       if (chunk > 0 && lane == 0) {
         unsigned long long t0 = 0;
         while (*(volatile int32_t*)(A.done + unit) < chunk) {
@@ -143,7 +149,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
           unsigned long long now;
           asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
           if (t0 == 0) t0 = now;
-          else if (now - t0 > 600ull * 1000000000ull) __trap();   // 10 min: fail loudly instead of hanging
+          else if (now - t0 > A.wait_budget_ns) __trap();         // fail loudly instead of hanging
         }
       }
       __syncwarp();
@@ -158,9 +164,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
       status = packed & 0xff;
       flag = (packed >> 8) & ST_NEWTON_FLAG;   // bit 16 -> 256
       frozen = packed < 0;
-      steps = __ldcg(A.carry_i + tp + t);
-      until_renorm = __ldcg(A.carry_i + 2 * tp + t);
-      gn_total = __ldcg(A.carry_g + t);
+      until_renorm = __ldcg(A.carry_i + tp + t);
     }
 
     // steps until the next sample; a countdown instead of a modulo in the step loop
@@ -200,7 +204,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
 #pragma unroll
           for (int i = 0; i < 12; ++i) y[i] = z[i];
           ++steps;
-          gn_total += (unsigned)gn;
+          gn_chunk += (unsigned)gn;
         } else {
           frozen = true;
           status = code;
@@ -244,6 +248,13 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
     }
 
     const bool last = chunk + 1 == A.n_chunks;
+    const bool carried = chunk > 0 || A.resume;
+    unsigned long long gn_total = gn_chunk;
+    long long steps_total = steps;
+    if (carried) {
+      gn_total += __ldcg(A.carry_g + t);
+      steps_total += (long long)__ldcg(A.carry_g + tp + t);
+    }
     if (!last || A.save_final) {
       // park the state in the carry buffer (and publish the chunk unless it is the last)
 #pragma unroll
@@ -253,13 +264,14 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
       for (int i = 0; i < 3; ++i) __stcg(A.carry_d + (int64_t)(13 + i) * tp + t, R.J0[i]);
       __stcg(A.carry_d + 16 * tp + t, acc);
       __stcg(A.carry_i + t, (status & 0xff) | (flag << 8) | (frozen ? (int)0x80000000 : 0));
-      __stcg(A.carry_i + tp + t, steps);
-      __stcg(A.carry_i + 2 * tp + t, until_renorm);
+      __stcg(A.carry_i + tp + t, until_renorm);
       __stcg(A.carry_g + t, gn_total);
+      __stcg(A.carry_g + tp + t, (unsigned long long)steps_total);
       if (!last) {
-        __threadfence();
+        // publish: the barrier collects every lane's st.cg, then the lane that writes the flag issues the release
+        // fence (cumulativity: it covers the stores it observed through the barrier) and the flag store
         __syncwarp();
-        if (lane == 0) atomicExch(A.done + unit, chunk + 1);
+        if (lane == 0) { __threadfence(); atomicExch(A.done + unit, chunk + 1); }
         continue;
       }
     }
@@ -287,7 +299,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
         for (int i = 0; i < 6; ++i) A.out_inv[(int64_t)(6 + i) * A.n + orbit] = inv1[i];
       }
       A.out_status[orbit] = status | flag;
-      A.out_step[orbit] = steps;
+      A.out_step[orbit] = steps_total;
       A.out_gn[orbit] = (int64_t)gn_total;
     }
   }

@@ -1,11 +1,23 @@
-// mc_math.cuh -- per-trajectory device math: fused Hamiltonian / gradient / precession routine,
-// classical RK4, correction operators.  Everything lives in registers; one thread = one trajectory.
+// mc_math.cuh -- per-trajectory math: fused Hamiltonian / gradient / precession routine, classical RK4,
+// Butcher RK5.  Everything lives in registers; one thread = one trajectory.
 //
 // Formulation: unit spins, raw dot products (no unit vector n), all inverse
 // powers of r from one rsqrt, Horner polynomials in P = p.p, Q = (n.p)^2, u = 1/r, FMA-first.
 // The oracle (oracle/pn_oracle.hpp) is written differently on purpose; the two share no code.
+//
+// Every routine is a template on the scalar type T.  The kernels use T = double.  The host-only flop model
+// (mc_flop_model.cpp, plain C++) instantiates the very same routines with T = mc::Cnt, a scalar that counts
+// its own FMAs, multiplications, additions and special functions -- so the algorithmic flop figures bench.py
+// reports are derived from the code that runs, not from a hand count.
 #pragma once
 #include "mc_consts.h"
+
+#ifdef __CUDACC__
+#define MC_DEV __device__ __forceinline__
+#else
+#include <cmath>
+#define MC_DEV inline
+#endif
 
 namespace mc {
 
@@ -15,25 +27,15 @@ namespace mc {
 // shared memory, laid out [MC_NCONST][blockDim.x] (conflict-free LDS.64).
 struct UniformConsts {
   const McConsts& k;
-  __device__ __forceinline__ double operator[](int i) const { return k.v[i]; }
+  MC_DEV double operator[](int i) const { return k.v[i]; }
 };
 struct SharedConsts {
   const double* base;  // &smem[threadIdx.x]
   int stride;          // blockDim.x
-  __device__ __forceinline__ double operator[](int i) const { return base[i * stride]; }
+  MC_DEV double operator[](int i) const { return base[i * stride]; }
 };
 
-// ---- small helpers ------------------------------------------------------------------------------
-__device__ __forceinline__ double dot3(const double* a, const double* b) {
-  return fma(a[2], b[2], fma(a[1], b[1], a[0] * b[0]));
-}
-// c = a x b
-__device__ __forceinline__ void cross3(const double* a, const double* b, double* c) {
-  c[0] = fma(a[1], b[2], -(a[2] * b[1]));
-  c[1] = fma(a[2], b[0], -(a[0] * b[2]));
-  c[2] = fma(a[0], b[1], -(a[1] * b[0]));
-}
-
+#ifdef __CUDACC__
 // 1/sqrt(x) for x > 0, normal: MUFU.RSQ64H seed (~2^-22 relative) + one third-order step
 // y <- y (1 + e/2 + 3 e^2/8), e = 1 - x y^2  => relative error ~ 1e-20 before rounding.
 __device__ __forceinline__ double rsqrt_pos(double x) {
@@ -53,6 +55,9 @@ __device__ __forceinline__ double rcp_nz(double x) {
   e = fma(-x, y, 1.0);
   return fma(y, e, y);
 }
+__device__ __forceinline__ double sqrt_pos(double x) { return sqrt(x); }
+__device__ __forceinline__ double div_(double a, double b) { return a / b; }
+__device__ __forceinline__ bool is_finite(double v) { return (((unsigned)__double2hiint(v)) & 0x7ff00000u) != 0x7ff00000u; }
 
 __device__ __forceinline__ bool finite12(const double* z) {
   // exponent field all ones <=> inf or nan <=> (high word with the sign shifted out) >= 0xffe00000.  Integer pipe
@@ -64,79 +69,93 @@ __device__ __forceinline__ bool finite12(const double* z) {
   const unsigned c = max(max(m[6], m[7]), m[8]), d = max(max(m[9], m[10]), m[11]);
   return max(max(a, b), max(c, d)) < 0xffe00000u;
 }
+#endif
+
+// ---- small helpers ------------------------------------------------------------------------------
+template <class T>
+MC_DEV T dot3(const T* a, const T* b) {
+  return fma(a[2], b[2], fma(a[1], b[1], a[0] * b[0]));
+}
+// c = a x b
+template <class T>
+MC_DEV void cross3(const T* a, const T* b, T* c) {
+  c[0] = fma(a[1], b[2], -(a[2] * b[1]));
+  c[1] = fma(a[2], b[0], -(a[0] * b[2]));
+  c[2] = fma(a[0], b[1], -(a[1] * b[0]));
+}
 
 // ---- the fused model routine ----------------------------------------------------------------------
 // Input  z = (r[0:3], p[3:6], sigma1[6:9], sigma2[9:12]).
 // Output g[0:3] = dH/dr, g[3:6] = dH/dp; if OMEGA: g[6:9] = Omega1, g[9:12] = Omega2; if WANT_H: H.
 // eqs (1)-(9) of the paper with the readings of DESIGN.md section 3.
-template <bool QM, bool OMEGA, bool WANT_H, class C>
-__device__ __forceinline__ void pn_eval(const C& c, const double* z, double* g, double& H) {
-  const double* r = z;
-  const double* p = z + 3;
-  const double* s1 = z + 6;
-  const double* s2 = z + 9;
-  const double r2 = dot3(r, r);
-  const double u = rsqrt_pos(r2);
-  const double u2 = u * u, u3 = u2 * u, u5 = u3 * u2;
-  const double rp = dot3(r, p);
-  const double P = dot3(p, p);
-  const double w = rp * u2;                                        // (n.p) u
-  const double Q = rp * w;                                         // (n.p)^2
+template <bool QM, bool OMEGA, bool WANT_H, class C, class T>
+MC_DEV void pn_eval(const C& c, const T* z, T* g, T& H) {
+  const T* r = z;
+  const T* p = z + 3;
+  const T* s1 = z + 6;
+  const T* s2 = z + 9;
+  const T r2 = dot3(r, r);
+  const T u = rsqrt_pos(r2);
+  const T u2 = u * u, u3 = u2 * u, u5 = u3 * u2;
+  const T rp = dot3(r, p);
+  const T P = dot3(p, p);
+  const T w = rp * u2;                                        // (n.p) u
+  const T Q = rp * w;                                         // (n.p)^2
 
   // orbital polynomials (Horner); every constant multiple is precomputed (mc_consts.h)
-  const double t1 = fma(c[K_D2], Q, fma(c[K_D1], P, c[K_B1]));   // b1 + d1 P + d2 Q
-  const double t2 = fma(c[K_D3], Q, c[K_B2]);                    // b2 + d3 Q
-  const double t3 = WANT_H ? fma(c[K_E2], Q, c[K_E1] * P) : 0.0;  // e1 P + e2 Q (only H itself needs it)
+  const T t1 = fma(c[K_D2], Q, fma(c[K_D1], P, c[K_B1]));   // b1 + d1 P + d2 Q
+  const T t2 = fma(c[K_D3], Q, c[K_B2]);                    // b2 + d3 Q
+  const T t3 = WANT_H ? fma(c[K_E2], Q, c[K_E1] * P) : T(0.0);  // e1 P + e2 Q (only H itself needs it)
   // H_P = 1/2 + P (2 a1 + 3 c3 P) + u (b1 + 2 d1 P + d2 Q + e1 u)
-  const double hp_u = fma(c[K_E1], u, fma(c[K_D1], P, t1));
-  const double HP = fma(u, hp_u, fma(P, fma(c[K_3C3], P, c[K_2A1]), 0.5));
+  const T hp_u = fma(c[K_E1], u, fma(c[K_D1], P, t1));
+  const T HP = fma(u, hp_u, fma(P, fma(c[K_3C3], P, c[K_2A1]), 0.5));
   // 2 H_Q = u (2 b2 + 2 d2 P + 4 d3 Q + 2 e2 u)
-  const double HQ2 = u * fma(c[K_4D3], Q, fma(c[K_2D2], P, fma(c[K_2E2], u, c[K_2B2])));
+  const T HQ2 = u * fma(c[K_4D3], Q, fma(c[K_2D2], P, fma(c[K_2E2], u, c[K_2B2])));
   // H_u = -1 + P t1 + Q t2 + u (2 h1 + 2 t3 + 3 f1 u)
-  const double hu_u = WANT_H ? fma(c[K_3F1], u, fma(2.0, t3, c[K_2H1]))
-                             : fma(c[K_3F1], u, fma(c[K_2E1], P, fma(c[K_2E2], Q, c[K_2H1])));
-  const double Hu = fma(u, hu_u, fma(Q, t2, fma(P, t1, -1.0)));
-  const double A = HP + HP;                                // dH_orb/dp = A p + B r
-  const double B = HQ2 * w;
-  const double Cu = fma(Hu, u, HQ2 * Q);                   // dH_orb/dr = B p - u^2 Cu r
+  const T hu_u = WANT_H ? fma(c[K_3F1], u, fma(2.0, t3, c[K_2H1]))
+                        : fma(c[K_3F1], u, fma(c[K_2E1], P, fma(c[K_2E2], Q, c[K_2H1])));
+  const T Hu = fma(u, hu_u, fma(Q, t2, fma(P, t1, -1.0)));
+  const T A = HP + HP;                                // dH_orb/dp = A p + B r
+  const T B = HQ2 * w;
+  const T Cu = fma(Hu, u, HQ2 * Q);                   // dH_orb/dr = B p - u^2 Cu r
 
   // spin couplings
-  const double a1 = dot3(s1, r), a2 = dot3(s2, r), d12 = dot3(s1, s2);
-  const double k1u = c[K_K1] * u3, k2u = c[K_K2] * u3;
-  double Sg[3], L[3], SxR[3], PxS[3];
+  const T a1 = dot3(s1, r), a2 = dot3(s2, r), d12 = dot3(s1, s2);
+  const T k1u = c[K_K1] * u3, k2u = c[K_K2] * u3;
+  T Sg[3], L[3], SxR[3], PxS[3];
 #pragma unroll
   for (int i = 0; i < 3; ++i) Sg[i] = fma(k2u, s2[i], k1u * s1[i]);   // u^3 (k1 sigma1 + k2 sigma2)
   cross3(r, p, L);
   cross3(Sg, r, SxR);
   cross3(p, Sg, PxS);
-  const double LS = dot3(L, Sg);                                      // = H_SO
-  const double a12u5 = a1 * a2 * u5;
-  const double c12u3 = c[K_C12] * u3;
+  const T LS = dot3(L, Sg);                                      // = H_SO
+  const T a12u5 = a1 * a2 * u5;
+  const T c12u3 = c[K_C12] * u3;
   // coefficient of r in dH_spin/dr is 3 u^2 X:  X = -H_SO + c12 (d12 u^3 - 5 a1 a2 u^5) + QM
-  double X = fma(c12u3, d12, fma(c[K_M5C12], a12u5, -LS));
-  const double c12u5x3 = c[K_3C12] * u5;
-  double w1 = c12u5x3 * a2, w2 = c12u5x3 * a1;
-  double Hss = fma(c[K_3C12], a12u5, -(c12u3 * d12));
+  T X = fma(c12u3, d12, fma(c[K_M5C12], a12u5, -LS));
+  const T c12u5x3 = c[K_3C12] * u5;
+  T w1 = c12u5x3 * a2, w2 = c12u5x3 * a1;
+  T Hss = fma(c[K_3C12], a12u5, -(c12u3 * d12));
   if (QM) {
-    const double d11 = dot3(s1, s1), d22 = dot3(s2, s2);
-    const double q1u3 = c[K_Q1] * u3, q2u3 = c[K_Q2] * u3;
-    const double a11u5 = a1 * a1 * u5, a22u5 = a2 * a2 * u5;
+    const T d11 = dot3(s1, s1), d22 = dot3(s2, s2);
+    const T q1u3 = c[K_Q1] * u3, q2u3 = c[K_Q2] * u3;
+    const T a11u5 = a1 * a1 * u5, a22u5 = a2 * a2 * u5;
     X = fma(q1u3, d11, fma(-5.0 * c[K_Q1], a11u5, X));
     X = fma(q2u3, d22, fma(-5.0 * c[K_Q2], a22u5, X));
     w1 = fma(6.0 * c[K_Q1] * u5, a1, w1);
     w2 = fma(6.0 * c[K_Q2] * u5, a2, w2);
     Hss += fma(3.0 * c[K_Q1], a11u5, -(q1u3 * d11)) + fma(3.0 * c[K_Q2], a22u5, -(q2u3 * d22));
   }
-  const double Cr = u2 * fma(3.0, X, -Cu);                 // coefficient of r in dH/dr
+  const T Cr = u2 * fma(3.0, X, -Cu);                 // coefficient of r in dH/dr
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
     g[i] = fma(w2, s2[i], fma(w1, s1[i], fma(Cr, r[i], fma(B, p[i], PxS[i]))));
     g[3 + i] = fma(A, p[i], fma(B, r[i], SxR[i]));
   }
   if (OMEGA) {
-    const double o1u = c[K_O1] * u3, o2u = c[K_O2] * u3;
-    const double m12u = c[K_M12] * u3, m21u = c[K_M21] * u3;
-    double b1r = c[K_3M12] * a2, b2r = c[K_3M21] * a1;
+    const T o1u = c[K_O1] * u3, o2u = c[K_O2] * u3;
+    const T m12u = c[K_M12] * u3, m21u = c[K_M21] * u3;
+    T b1r = c[K_3M12] * a2, b2r = c[K_3M21] * a1;
     if (QM) { b1r = fma(3.0 * c[K_M11], a1, b1r); b2r = fma(3.0 * c[K_M22], a2, b2r); }
     b1r *= u5;
     b2r *= u5;
@@ -148,15 +167,15 @@ __device__ __forceinline__ void pn_eval(const C& c, const double* z, double* g, 
   }
   if (WANT_H) {
     // H = P/2 - u + P^2 (a1 + c3 P) + u (P t1 + Q t2) + u^2 (h1 + t3) + f1 u^3 + H_SO + H_SS
-    const double orb = fma(u2, fma(c[K_F1], u, c[K_H1] + t3), fma(u, fma(Q, t2, P * t1), fma(P * P, fma(c[K_C3], P, c[K_A1]), fma(0.5, P, -u))));
+    const T orb = fma(u2, fma(c[K_F1], u, c[K_H1] + t3), fma(u, fma(Q, t2, P * t1), fma(P * P, fma(c[K_C3], P, c[K_A1]), fma(0.5, P, -u))));
     H = orb + (LS + Hss);
   }
 }
 
 // dz/dt, eqs (6)-(7): dr/dt = dH/dp, dp/dt = -dH/dr, dsigma_i/dt = Omega_i x sigma_i.
-template <bool QM, class C>
-__device__ __forceinline__ void pn_rhs(const C& c, const double* z, double* f) {
-  double g[12], H;
+template <bool QM, class C, class T>
+MC_DEV void pn_rhs(const C& c, const T* z, T* f) {
+  T g[12], H;
   pn_eval<QM, true, false>(c, z, g, H);
 #pragma unroll
   for (int i = 0; i < 3; ++i) { f[i] = g[3 + i]; f[3 + i] = -g[i]; }
@@ -165,25 +184,25 @@ __device__ __forceinline__ void pn_rhs(const C& c, const double* z, double* f) {
 }
 
 // J = r x p + s1 sigma1 + s2 sigma2
-template <class C>
-__device__ __forceinline__ void total_J(const C& c, const double* z, double* J) {
+template <class C, class T>
+MC_DEV void total_J(const C& c, const T* z, T* J) {
   cross3(z, z + 3, J);
 #pragma unroll
   for (int i = 0; i < 3; ++i) J[i] = fma(c[K_S2], z[9 + i], fma(c[K_S1], z[6 + i], J[i]));
 }
 
-template <bool QM, class C>
-__device__ __forceinline__ double hamiltonian(const C& c, const double* z) {
-  double g[12], H;
+template <bool QM, class C, class T>
+MC_DEV T hamiltonian(const C& c, const T* z) {
+  T g[12], H;
   pn_eval<QM, false, true>(c, z, g, H);
   return H;
 }
 
 // Classical RK4 (R9), low-storage bookkeeping: y (kept), acc, stage input yt.
-template <bool QM, class C>
-__device__ __forceinline__ void rk4_step(const C& c, const double* y, double h, double* out) {
+template <bool QM, class C, class T>
+MC_DEV void rk4_step(const C& c, const T* y, double h, T* out) {
   const double h2 = 0.5 * h, h3 = h * (1.0 / 3.0), h6 = h * (1.0 / 6.0);
-  double k[12], yt[12];
+  T k[12], yt[12];
   pn_rhs<QM>(c, y, k);
 #pragma unroll
   for (int i = 0; i < 12; ++i) { out[i] = fma(h6, k[i], y[i]); yt[i] = fma(h2, k[i], y[i]); }
@@ -203,9 +222,9 @@ __device__ __forceinline__ void rk4_step(const C& c, const double* y, double h, 
 //   a2 = (1/4); a3 = (1/8, 1/8); a4 = (0, -1/2, 1); a5 = (3/16, 0, 0, 9/16); a6 = (-3/7, 2/7, 12/7, -12/7, 8/7)
 // Bookkeeping: the linear combinations needed later (stage-4 input, stage-6 input, final sum) are accumulated as
 // the stages arrive, so at most five 12-vectors are live besides the derivative being computed.
-template <bool QM, class C>
-__device__ __forceinline__ void rk5_step(const C& c, const double* y, double h, double* out) {
-  double k[12], k1[12], yt[12], A4[12], S6[12];
+template <bool QM, class C, class T>
+MC_DEV void rk5_step(const C& c, const T* y, double h, T* out) {
+  T k[12], k1[12], yt[12], A4[12], S6[12];
   pn_rhs<QM>(c, y, k1);
   const double h4 = 0.25 * h, h8 = 0.125 * h;
 #pragma unroll
@@ -247,15 +266,16 @@ __device__ __forceinline__ void rk5_step(const C& c, const double* y, double h, 
 }
 
 // INTEG: 0 classical RK4, 1 Butcher RK5
-template <int INTEG, bool QM, class C>
-__device__ __forceinline__ void base_step(const C& c, const double* y, double h, double* out) {
+template <int INTEG, bool QM, class C, class T>
+MC_DEV void base_step(const C& c, const T* y, double h, T* out) {
   if (INTEG == 1) rk5_step<QM>(c, y, h, out);
   else rk4_step<QM>(c, y, h, out);
 }
 
 // eq (10): sigma <- sigma / |sigma|
-__device__ __forceinline__ void normalise3(double* s) {
-  const double w = rsqrt_pos(dot3(s, s));
+template <class T>
+MC_DEV void normalise3(T* s) {
+  const T w = rsqrt_pos(dot3(s, s));
   s[0] *= w; s[1] *= w; s[2] *= w;
 }
 

@@ -1,23 +1,43 @@
-"""Host-side logic of the multi-GPU path: orbits are independent, so ranks own
-contiguous orbit-index ranges and no collective touches the data path.  The only communication is the
-max-over-ranks of each rank's device time (one scalar), which bench.py needs for the job throughput.
+"""Host-side logic of the multi-GPU path: orbits are independent, so every rank owns a
+fixed subset of the grid rows and no collective touches the data path.  Rows are dealt round-robin (global row i
+belongs to rank i mod N): the strong-field rows (small r0: dropped and chaotic cells, more Gauss-Newton steps) and
+the calm ones are then spread evenly, and since the job time is the maximum over ranks a contiguous split would
+measure the imbalance between the first and the last r0 band instead of the machine.  The only communication is
+the max-over-ranks of each rank's device time (one scalar), which bench.py needs for the job throughput.
 
 Backend-agnostic (nccl on GPUs, gloo in the CPU tests): tensors are created on the device passed in.
 """
 import numpy as np
 
-from .workloads import Workload, shard_range
+from .workloads import Workload
 
 
-def rank_rows(n_rows_per_rank: int, rank: int, world_size: int):
-    """Row range [lo, hi) of a grid widened to n_rows_per_rank * world_size rows (weak scaling)."""
-    return shard_range(n_rows_per_rank * world_size, rank, world_size)
+def rank_rows(n_rows_per_rank: int, rank: int, world_size: int) -> np.ndarray:
+    """Global row indices of `rank` in a grid widened to n_rows_per_rank * world_size rows (weak scaling):
+    rank, rank + N, rank + 2N, ... (round-robin)."""
+    return np.arange(rank, n_rows_per_rank * world_size, world_size)
+
+
+def rank_orbits(n_rows_per_rank: int, n_cols: int, rank: int, world_size: int) -> np.ndarray:
+    """Global orbit indices (row-major, index = row * n_cols + col) of `rank`, in the order it integrates them."""
+    rows = rank_rows(n_rows_per_rank, rank, world_size)
+    return (rows[:, None] * n_cols + np.arange(n_cols)[None, :]).ravel()
 
 
 def rank_shard(w: Workload, n_rows_per_rank: int, n_cols: int, rank: int, world_size: int) -> Workload:
-    """The slice of a row-major (rows x n_cols) grid workload that `rank` integrates."""
-    lo, hi = rank_rows(n_rows_per_rank, rank, world_size)
-    return w.subset(np.arange(lo * n_cols, hi * n_cols))
+    """The part of a row-major (rows x n_cols) grid workload that `rank` integrates."""
+    return w.subset(rank_orbits(n_rows_per_rank, n_cols, rank, world_size))
+
+
+def scatter_back(parts, n_rows_per_rank: int, n_cols: int, world_size: int) -> np.ndarray:
+    """Inverse of the split for an output array: parts[r] has the rank-local orbit axis last; returns the global
+    array (outputs of different ranks are disjoint slices, so this is a permutation, not a reduction)."""
+    n = n_rows_per_rank * world_size * n_cols
+    first = np.asarray(parts[0])
+    out = np.empty(first.shape[:-1] + (n,), dtype=first.dtype)
+    for r, part in enumerate(parts):
+        out[..., rank_orbits(n_rows_per_rank, n_cols, r, world_size)] = np.asarray(part)
+    return out
 
 
 def max_over_ranks(value: float, device=None) -> float:

@@ -70,7 +70,10 @@ typedef struct mc_params {
   uint32_t struct_size;   /* = sizeof(mc_params); checked by mc_create                                   */
   uint32_t terms;         /* OR of mc_terms                                                              */
   int32_t device;         /* CUDA device ordinal                                                         */
-  int32_t per_orbit;      /* 0: the five scalars below apply to every orbit; 1: use the device arrays      */
+  int32_t per_orbit;      /* 0: the five scalars below apply to every orbit; 1: use the five device arrays;
+                             2: beta, chi1, chi2 scalars for every orbit, kq1, kq2 per orbit from d_kq1, d_kq2
+                             (BASELINE config 3: one binary model, a scan over quadrupole coefficients) -- the
+                             constants that do not depend on kq stay constant-bank operands of the kernel      */
   double beta;            /* mass ratio m1/m2 in (0,1]                                       */
   double chi1, chi2;      /* dimensionless spins in [0,1]                                   */
   double kq1, kq2;        /* quadrupole coefficients, 1 = black hole (R16)         */
@@ -195,7 +198,7 @@ typedef struct mc_launch_info {
   int32_t blocks_per_sm;        /* occupancy API result for that block size       */
   int32_t num_sms;
   int32_t smem_bytes;           /* dynamic shared memory per block                */
-  int32_t variant;              /* bit0 per-orbit params, bit1 QM, bits 4-5 mode, bit 8 RK5 */
+  int32_t variant;              /* bit0 per-orbit params, bit1 QM, bit2 per-orbit kq only, bits 4-5 mode, bit 8 RK5 */
   int64_t trajectories;         /* threads doing work = n_orbits * (1 + shadow)   */
   int32_t chunk_steps;          /* steps per work item                             */
   int32_t n_chunks;             /* work items per 32-trajectory unit              */

@@ -155,7 +155,7 @@ class Integrator:
 
     def __init__(self, terms=TERMS_DEFAULT, beta=1.0, chi1=1.0, chi2=1.0, kq1=1.0, kq2=1.0, device=0,
                  renorm_interval=100, newton_iters=4, newton_tol=1e-10, r_merge=2.0, r_escape=1e4, stream=None,
-                 chunk_steps=0, integrator=0, wait_budget_s=600.0):
+                 chunk_steps=0, integrator=0, wait_budget_s=600.0, per_orbit=None):
         import torch
         self._torch = torch
         self._lib = load_library()
@@ -168,20 +168,42 @@ class Integrator:
         p.wait_budget_s = float(wait_budget_s)
         self.device = torch.device("cuda", device)
         vals = dict(beta=beta, chi1=chi1, chi2=chi2, kq1=kq1, kq2=kq2)
-        per_orbit = any(hasattr(v, "__len__") for v in vals.values())
+
+        def uniform_value(v):
+            """The scalar all orbits share, or None if the parameter really varies."""
+            if not hasattr(v, "__len__"):
+                return float(v)
+            import numpy as np
+            a = np.asarray(v, dtype=np.float64)
+            return float(a.flat[0]) if a.size and (a == a.flat[0]).all() else None
+
+        uni = {k: uniform_value(v) for k, v in vals.items()}
         self._keep = []
         self.n_params = None
-        if per_orbit:
-            n = max(len(v) for v in vals.values() if hasattr(v, "__len__"))
+        arrays = [k for k, u in uni.items() if u is None]
+        if per_orbit == 1:                               # forced: every parameter as a device array (tests)
+            arrays = [k for k, v in vals.items() if hasattr(v, "__len__")] + ["beta"]
+            uni = {k: None for k in vals}
+        if not arrays:                                   # mc_params.per_orbit = 0
+            for name, u in uni.items():
+                setattr(p, name, u)
+        elif set(arrays) <= {"kq1", "kq2"}:              # per_orbit = 2: one binary model, per-orbit quadrupole coefficients
+            self.n_params = max(len(vals[k]) for k in arrays)
+            p.per_orbit = 2
+            for name in ("beta", "chi1", "chi2"):
+                setattr(p, name, uni[name])
+            for name in ("kq1", "kq2"):
+                t = torch.as_tensor(vals[name], dtype=torch.float64).expand(self.n_params).contiguous().to(self.device)
+                self._keep.append(t)                     # must outlive the handle (include/mc.h)
+                setattr(p, "d_" + name, t.data_ptr())
+        else:                                            # per_orbit = 1
+            n = max([len(v) for v in vals.values() if hasattr(v, "__len__")] + [1])
             self.n_params = n
             p.per_orbit = 1
             for name, v in vals.items():
                 t = torch.as_tensor(v, dtype=torch.float64).expand(n).contiguous().to(self.device)
                 self._keep.append(t)            # must outlive the handle (include/mc.h)
                 setattr(p, "d_" + name, t.data_ptr())
-        else:
-            for name, v in vals.items():
-                setattr(p, name, float(v))
         if stream is None:
             stream = torch.cuda.current_stream(self.device)
         self.stream = stream

@@ -70,7 +70,7 @@ int valid_scalars(double beta, double chi1, double chi2, double kq1, double kq2)
 }
 
 // ---- evaluation kernel for mc_eval ---------------------------------------------------------------
-template <bool PER_ORBIT, bool QM>
+template <int PARAMS, bool QM>
 __global__ void __launch_bounds__(mc::kBlock)
 eval_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ mc::IntegrateArgs A, int what, int mode,
             const double* __restrict__ refs, double* __restrict__ out) {
@@ -78,15 +78,8 @@ eval_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ mc::Int
   const int64_t t = (int64_t)blockIdx.x * mc::kBlock + threadIdx.x;
   const bool active = t < A.n;
   const int64_t o = active ? t : A.n - 1;
-  using CP = typename std::conditional<PER_ORBIT, mc::SharedConsts, mc::UniformConsts>::type;
-  CP c = [&]() {
-    if constexpr (PER_ORBIT) {
-      mc_derive_consts(A.beta[o], A.chi1[o], A.chi2[o], A.kq1[o], A.kq2[o], A.terms, smem + threadIdx.x, mc::kBlock);
-      return mc::SharedConsts{smem + threadIdx.x, mc::kBlock};
-    } else {
-      return mc::UniformConsts{uc};
-    }
-  }();
+  using CP = typename mc::ConstsOf<PARAMS>::type;
+  const CP c = mc::make_consts<PARAMS, CP>(uc, A, o, smem);
   double z[12], f[12];
 #pragma unroll
   for (int i = 0; i < 12; ++i) z[i] = A.states[(int64_t)i * A.n + o];
@@ -187,8 +180,11 @@ int mc_create(const mc_params* params, mc_handle** out_handle) {
   if (params->integrator != MC_INTEG_RK4 && params->integrator != MC_INTEG_RK5) return MC_EINVAL;
   if (!(params->newton_tol >= 0.0) || !(params->r_merge >= 0.0) || !(params->r_escape > params->r_merge)) return MC_EINVAL;
   if (!(params->wait_budget_s > 0.0) || !(params->wait_budget_s <= 1e9)) return MC_EINVAL;
-  if (params->per_orbit) {
+  if (params->per_orbit < 0 || params->per_orbit > 2) return MC_EINVAL;
+  if (params->per_orbit == 1) {
     if (!params->d_beta || !params->d_chi1 || !params->d_chi2 || !params->d_kq1 || !params->d_kq2) return MC_EINVAL;
+  } else if (params->per_orbit == 2) {
+    if (!params->d_kq1 || !params->d_kq2 || !valid_scalars(params->beta, params->chi1, params->chi2, 1.0, 1.0)) return MC_EINVAL;
   } else if (!valid_scalars(params->beta, params->chi1, params->chi2, params->kq1, params->kq2)) {
     return MC_EINVAL;
   }
@@ -206,7 +202,9 @@ int mc_create(const mc_params* params, mc_handle** out_handle) {
   h->num_sms = prop.multiProcessorCount;
   h->last_n = 0;
   memset(&h->info, 0, sizeof(h->info));
-  if (params->per_orbit) memset(&h->uc, 0, sizeof(h->uc));
+  if (params->per_orbit == 1) memset(&h->uc, 0, sizeof(h->uc));
+  else if (params->per_orbit == 2)   // the kappa-dependent constants (q_i, m_ii) are linear in kappa: derived with kappa = 1
+    mc_derive_consts(params->beta, params->chi1, params->chi2, 1.0, 1.0, params->terms, h->uc.v);
   else mc_derive_consts(params->beta, params->chi1, params->chi2, params->kq1, params->kq2, params->terms, h->uc.v);
   *out_handle = h;
   return MC_OK;
@@ -276,10 +274,10 @@ static int integrate_impl(mc_handle* h, const double* states, int64_t n_orbits, 
   const bool qm = (h->P.terms & MC_TERM_QM) != 0;
   mc::LaunchFn fn = nullptr;
   switch (correction_mode) {
-    case 0: fn = mc::launcher_mode0(h->P.per_orbit != 0, qm, h->P.integrator); break;
-    case 1: fn = mc::launcher_mode1(h->P.per_orbit != 0, qm, h->P.integrator); break;
-    case 2: fn = mc::launcher_mode2(h->P.per_orbit != 0, qm, h->P.integrator); break;
-    default: fn = mc::launcher_mode3(h->P.per_orbit != 0, qm, h->P.integrator); break;
+    case 0: fn = mc::launcher_mode0(h->P.per_orbit, qm, h->P.integrator); break;
+    case 1: fn = mc::launcher_mode1(h->P.per_orbit, qm, h->P.integrator); break;
+    case 2: fn = mc::launcher_mode2(h->P.per_orbit, qm, h->P.integrator); break;
+    default: fn = mc::launcher_mode3(h->P.per_orbit, qm, h->P.integrator); break;
   }
   const int64_t traj = n_orbits * (shadow ? 2 : 1);
   A.n_units = (traj + 31) / 32;
@@ -334,7 +332,8 @@ static int integrate_impl(mc_handle* h, const double* states, int64_t n_orbits, 
   h->info.blocks_per_sm = ki.blocks_per_sm;
   h->info.num_sms = h->num_sms;
   h->info.smem_bytes = (int32_t)ki.smem;
-  h->info.variant = (h->P.per_orbit ? 1 : 0) | (qm ? 2 : 0) | (correction_mode << 4) | (h->P.integrator << 8);
+  const int kparams = (h->P.per_orbit == 2 && !qm) ? 0 : h->P.per_orbit;   // kappa is unused without the QM term
+  h->info.variant = (kparams == 1 ? 1 : 0) | (qm ? 2 : 0) | (kparams == 2 ? 4 : 0) | (correction_mode << 4) | (h->P.integrator << 8);
   h->info.trajectories = traj;
   return MC_OK;
 }
@@ -396,13 +395,14 @@ int mc_eval(mc_handle* h, int32_t what, const double* states, int64_t n, double 
   mc::IntegrateArgs A;
   fill_args(h, A);
   A.states = states; A.n = n; A.h = step_h;
-  const bool qm = (h->P.terms & MC_TERM_QM) != 0, po = h->P.per_orbit != 0;
+  const bool qm = (h->P.terms & MC_TERM_QM) != 0, po = h->P.per_orbit == 1, ka = h->P.per_orbit == 2 && qm;
   const int grid = (int)((n + mc::kBlock - 1) / mc::kBlock);
   const size_t smem = po ? sizeof(double) * MC_NCONST * mc::kBlock : 0;
-  if (po && qm) eval_kernel<true, true><<<grid, mc::kBlock, smem, h->stream>>>(h->uc, A, what, mode, refs, out);
-  else if (po) eval_kernel<true, false><<<grid, mc::kBlock, smem, h->stream>>>(h->uc, A, what, mode, refs, out);
-  else if (qm) eval_kernel<false, true><<<grid, mc::kBlock, smem, h->stream>>>(h->uc, A, what, mode, refs, out);
-  else eval_kernel<false, false><<<grid, mc::kBlock, smem, h->stream>>>(h->uc, A, what, mode, refs, out);
+  if (po && qm) eval_kernel<1, true><<<grid, mc::kBlock, smem, h->stream>>>(h->uc, A, what, mode, refs, out);
+  else if (po) eval_kernel<1, false><<<grid, mc::kBlock, smem, h->stream>>>(h->uc, A, what, mode, refs, out);
+  else if (ka) eval_kernel<2, true><<<grid, mc::kBlock, smem, h->stream>>>(h->uc, A, what, mode, refs, out);
+  else if (qm) eval_kernel<0, true><<<grid, mc::kBlock, smem, h->stream>>>(h->uc, A, what, mode, refs, out);
+  else eval_kernel<0, false><<<grid, mc::kBlock, smem, h->stream>>>(h->uc, A, what, mode, refs, out);
   MC_CUDA(cudaGetLastError());
   return MC_OK;
 }

@@ -77,10 +77,31 @@ __device__ __forceinline__ void six_integrals(const C& c, const double* z, doubl
 #define MC_KERNEL_BOUNDS(MINB) __launch_bounds__(kBlock, MINB)
 #endif
 
-template <bool PER_ORBIT, bool QM, int MODE, int INTEG, int MINB>
+// PARAMS: 0 uniform parameters (constant bank), 1 every parameter per orbit (derived constants in shared memory),
+// 2 uniform beta, chi with per-orbit quadrupole coefficients (KappaConsts; instantiated with QM only).
+enum { PARAMS_UNIFORM = 0, PARAMS_PER_ORBIT = 1, PARAMS_KAPPA = 2 };
+
+template <int PARAMS, class CP>
+__device__ __forceinline__ CP make_consts(const McConsts& uc, const IntegrateArgs& A, int64_t orbit, double* smem) {
+  if constexpr (PARAMS == PARAMS_PER_ORBIT) {
+    mc_derive_consts(A.beta[orbit], A.chi1[orbit], A.chi2[orbit], A.kq1[orbit], A.kq2[orbit], A.terms,
+                     smem + threadIdx.x, kBlock);
+    return SharedConsts{smem + threadIdx.x, kBlock};
+  } else if constexpr (PARAMS == PARAMS_KAPPA) {
+    const double k1 = A.kq1[orbit], k2 = A.kq2[orbit];
+    return KappaConsts{uc, k1 * uc.v[K_Q1], k2 * uc.v[K_Q2], k1 * uc.v[K_3M11], k2 * uc.v[K_3M22]};
+  } else {
+    return UniformConsts{uc};
+  }
+}
+template <int PARAMS> struct ConstsOf { typedef UniformConsts type; };
+template <> struct ConstsOf<PARAMS_PER_ORBIT> { typedef SharedConsts type; };
+template <> struct ConstsOf<PARAMS_KAPPA> { typedef KappaConsts type; };
+
+template <int PARAMS, bool QM, int MODE, int INTEG, int MINB>
 __global__ void MC_KERNEL_BOUNDS(MINB)
 integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ IntegrateArgs A) {
-  extern __shared__ double smem[];   // PER_ORBIT: [MC_NCONST][kBlock]
+  extern __shared__ double smem[];   // PARAMS_PER_ORBIT: [MC_NCONST][kBlock]
   const bool shadow = A.shadow_eps != 0.0;
   const int lane = threadIdx.x & 31;
   const int64_t tp = A.n_units * 32;   // padded trajectory count = stride of the carry arrays
@@ -101,16 +122,8 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
     const bool active = orbit_raw < A.n;
     const int64_t orbit = active ? orbit_raw : (A.n - 1);   // idle lanes shadow-compute a valid orbit, never store
 
-    using CP = typename std::conditional<PER_ORBIT, SharedConsts, UniformConsts>::type;
-    CP c = [&]() {
-      if constexpr (PER_ORBIT) {
-        mc_derive_consts(A.beta[orbit], A.chi1[orbit], A.chi2[orbit], A.kq1[orbit], A.kq2[orbit], A.terms,
-                         smem + threadIdx.x, kBlock);
-        return SharedConsts{smem + threadIdx.x, kBlock};
-      } else {
-        return UniformConsts{uc};
-      }
-    }();
+    using CP = typename ConstsOf<PARAMS>::type;
+    const CP c = make_consts<PARAMS, CP>(uc, A, orbit, smem);
 
     double y[12];
     Refs R;

@@ -7,10 +7,11 @@
 
 namespace mc {
 
-// Resident 128-thread blocks per SM the register allocator must allow.  Uniform parameters are
-// constant-bank operands, so 3 blocks (<= 168 registers) fit without spills; per-orbit parameters, the
-// quadrupole-monopole term and the six-stage RK5 need <= 255 registers (2 blocks; within 6 % of the 3-block
-// speed, profiles/r01_config_sweep.md).  ptxas -v: 0 spill bytes for all 32 instantiations (checked by build()).
+// Resident 128-thread blocks per SM the register allocator must allow.  With constant-bank parameters (uniform, or
+// uniform + per-orbit kappa in four registers) the RK4 kernels fit 3 blocks (<= 168 registers) without spills, with
+// or without the quadrupole-monopole term.  Fully per-orbit parameters (37 constants in shared memory) and the
+// six-stage RK5 need <= 255 registers (2 blocks).  ptxas -v: 0 spill bytes for every instantiation (build() raises
+// otherwise).
 #ifndef MC_MINB_UNIFORM
 #define MC_MINB_UNIFORM 3
 #endif
@@ -18,11 +19,11 @@ namespace mc {
 #define MC_MINB_PER_ORBIT 2
 #endif
 
-template <bool PER_ORBIT, bool QM, int MODE, int INTEG>
+template <int PARAMS, bool QM, int MODE, int INTEG>
 static cudaError_t launch(const McConsts& uc, const IntegrateArgs& A, int num_sms, bool do_launch, cudaStream_t stream,
                           KernelInfo* info) {
-  auto kern = integrate_kernel<PER_ORBIT, QM, MODE, INTEG, ((PER_ORBIT || QM || INTEG == 1) ? MC_MINB_PER_ORBIT : MC_MINB_UNIFORM)>;
-  const size_t smem = PER_ORBIT ? sizeof(double) * MC_NCONST * kBlock : 0;
+  auto kern = integrate_kernel<PARAMS, QM, MODE, INTEG, ((PARAMS == PARAMS_PER_ORBIT || INTEG == 1) ? MC_MINB_PER_ORBIT : MC_MINB_UNIFORM)>;
+  const size_t smem = PARAMS == PARAMS_PER_ORBIT ? sizeof(double) * MC_NCONST * kBlock : 0;
   cudaFuncAttributes fa;
   cudaError_t e = cudaFuncGetAttributes(&fa, kern);
   if (e != cudaSuccess) return e;
@@ -45,15 +46,18 @@ static cudaError_t launch(const McConsts& uc, const IntegrateArgs& A, int num_sm
   return cudaGetLastError();
 }
 
+// params: 0 uniform, 1 per orbit, 2 per-orbit kappa only (meaningful with the QM term; without it kappa is unused
+// and the uniform kernel runs)
 template <int MODE, int INTEG>
-static LaunchFn pick2(bool per_orbit, bool qm) {
-  if (per_orbit) return qm ? launch<true, true, MODE, INTEG> : launch<true, false, MODE, INTEG>;
-  return qm ? launch<false, true, MODE, INTEG> : launch<false, false, MODE, INTEG>;
+static LaunchFn pick2(int params, bool qm) {
+  if (params == PARAMS_PER_ORBIT) return qm ? launch<PARAMS_PER_ORBIT, true, MODE, INTEG> : launch<PARAMS_PER_ORBIT, false, MODE, INTEG>;
+  if (params == PARAMS_KAPPA && qm) return launch<PARAMS_KAPPA, true, MODE, INTEG>;
+  return qm ? launch<PARAMS_UNIFORM, true, MODE, INTEG> : launch<PARAMS_UNIFORM, false, MODE, INTEG>;
 }
 
 template <int MODE>
-static LaunchFn pick(bool per_orbit, bool qm, int integrator) {
-  return integrator == 1 ? pick2<MODE, 1>(per_orbit, qm) : pick2<MODE, 0>(per_orbit, qm);
+static LaunchFn pick(int params, bool qm, int integrator) {
+  return integrator == 1 ? pick2<MODE, 1>(params, qm) : pick2<MODE, 0>(params, qm);
 }
 
 }  // namespace mc

@@ -34,6 +34,17 @@ struct SharedConsts {
   int stride;          // blockDim.x
   MC_DEV double operator[](int i) const { return base[i * stride]; }
 };
+// Uniform beta, chi1, chi2 with per-orbit quadrupole coefficients kappa_i (BASELINE config 3; mc_params.per_orbit
+// = 2): the constants that do not depend on kappa stay constant-bank operands, the four that do (q_i, 3 m_ii;
+// all linear in kappa_i) ride in registers.  i is a compile-time constant wherever this is called, so the
+// selection folds away.
+struct KappaConsts {
+  const McConsts& k;   // derived with kappa = 1
+  double q1, q2, m11x3, m22x3;
+  MC_DEV double operator[](int i) const {
+    return i == K_Q1 ? q1 : (i == K_Q2 ? q2 : (i == K_3M11 ? m11x3 : (i == K_3M22 ? m22x3 : k.v[i])));
+  }
+};
 
 #ifdef __CUDACC__
 // 1/sqrt(x) for x > 0, normal: MUFU.RSQ64H seed (~2^-22 relative) + one third-order step
@@ -137,14 +148,17 @@ MC_DEV void pn_eval(const C& c, const T* z, T* g, T& H) {
   T w1 = c12u5x3 * a2, w2 = c12u5x3 * a1;
   T Hss = fma(c[K_3C12], a12u5, -(c12u3 * d12));
   if (QM) {
+    // H_ii = q_i (3 a_i^2 u^5 - d_ii u^3).  Only q_i itself is used as a constant (no multiples), so that the
+    // per-orbit-kappa variant keeps one register per body; the numeric factors ride as FMA immediates.
     const T d11 = dot3(s1, s1), d22 = dot3(s2, s2);
     const T q1u3 = c[K_Q1] * u3, q2u3 = c[K_Q2] * u3;
-    const T a11u5 = a1 * a1 * u5, a22u5 = a2 * a2 * u5;
-    X = fma(q1u3, d11, fma(-5.0 * c[K_Q1], a11u5, X));
-    X = fma(q2u3, d22, fma(-5.0 * c[K_Q2], a22u5, X));
-    w1 = fma(6.0 * c[K_Q1] * u5, a1, w1);
-    w2 = fma(6.0 * c[K_Q2] * u5, a2, w2);
-    Hss += fma(3.0 * c[K_Q1], a11u5, -(q1u3 * d11)) + fma(3.0 * c[K_Q2], a22u5, -(q2u3 * d22));
+    const T q1a = q1u3 * u2 * a1, q2a = q2u3 * u2 * a2;        // q_i u^5 a_i
+    const T q1aa = q1a * a1, q2aa = q2a * a2;                  // q_i u^5 a_i^2
+    X = fma(q1u3, d11, fma(-5.0, q1aa, X));
+    X = fma(q2u3, d22, fma(-5.0, q2aa, X));
+    w1 = fma(6.0, q1a, w1);
+    w2 = fma(6.0, q2a, w2);
+    if (WANT_H) Hss += fma(3.0, q1aa, -(q1u3 * d11)) + fma(3.0, q2aa, -(q2u3 * d22));
   }
   const T Cr = u2 * fma(3.0, X, -Cu);                 // coefficient of r in dH/dr
 #pragma unroll
@@ -156,7 +170,7 @@ MC_DEV void pn_eval(const C& c, const T* z, T* g, T& H) {
     const T o1u = c[K_O1] * u3, o2u = c[K_O2] * u3;
     const T m12u = c[K_M12] * u3, m21u = c[K_M21] * u3;
     T b1r = c[K_3M12] * a2, b2r = c[K_3M21] * a1;
-    if (QM) { b1r = fma(3.0 * c[K_M11], a1, b1r); b2r = fma(3.0 * c[K_M22], a2, b2r); }
+    if (QM) { b1r = fma(c[K_3M11], a1, b1r); b2r = fma(c[K_3M22], a2, b2r); }
     b1r *= u5;
     b2r *= u5;
 #pragma unroll

@@ -116,3 +116,18 @@ def test_newton_iteration_stops_at_the_first_update_below_eps_times_p():
     # the discriminating case really sits between the two scales
     upd1 = np.linalg.norm(iterates[1][0:6] - zp[0:6], axis=0)
     assert (upd1 > 1e-3 * np.linalg.norm(zp[3:6], axis=0)).all() and (upd1 < 1e-3 * np.linalg.norm(zp[0:3], axis=0)).all()
+
+
+def test_conservative_runs_are_bit_identical_to_the_stored_oracle_outputs():
+    """tests/golden/oracle_conservative_regression.txt was written by the oracle (make_oracle_regression.py) before
+    any opt-in term was added to it; runs without the new term bits must reproduce it bit for bit."""
+    import importlib.util
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_oracle_regression", os.path.join(here, "make_oracle_regression.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    want = [l.rstrip("\n") for l in open(os.path.join(here, "oracle_conservative_regression.txt")) if not l.startswith("#")]
+    got = list(mod.lines())
+    assert len(want) == len(got) == 6 * len(mod.CASES)
+    assert got == want

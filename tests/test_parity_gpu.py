@@ -197,6 +197,46 @@ def test_config3_quadrupole_on_off_parity(mc):
     assert np.abs(out[True] - out[False]).max() > 1e-3          # the term really changes the dynamics
 
 
+def test_per_orbit_kappa_variant_matches_oracle_and_the_full_per_orbit_kernel(mc):
+    """mc_params.per_orbit = 2 (BASELINE config 3: one binary model, per-orbit quadrupole coefficients): the four
+    kappa-dependent constants ride in registers, everything else in the constant bank.  Model routines on random
+    states, then a shadowed run; the fully per-orbit kernel (per_orbit = 1) on the same inputs must agree with the
+    oracle to the same bar, and without the QM bit the library runs the uniform kernel (kappa is unused)."""
+    z = random_states(300, seed=21)
+    rng = np.random.default_rng(22)
+    par = dict(beta=0.8, chi1=0.9, chi2=0.7, kq1=rng.uniform(1, 8, 300), kq2=rng.uniform(1, 8, 300))
+    with mc.Integrator(terms=31, **par) as I:
+        assert I.params.per_orbit == 2
+        assert rel_state_err_blocks(I.eval("rhs", z).cpu().numpy(), oracle.rhs(z, terms=31, **par)) < 2e-13
+        assert np.abs(I.eval("H", z).cpu().numpy()[0] - oracle.hamiltonian(z, terms=31, **par)).max() < 1e-15
+        assert rel_state_err_blocks(I.eval("rk4_step", z, h=1.0).cpu().numpy(), oracle.rk4_step(z, 1.0, terms=31, **par)) < 2e-13
+    w = workloads.config3(n_r=12, n_theta=13, qm=True)
+    kw = {k: v for k, v in w.params().items() if k != "terms"}
+    o = oracle.integrate(w.states, 1.0, 1000, 3, shadow_eps=1e-8, **w.params())
+    ok = o.status == 0
+    got = {}
+    for force in (None, 1):
+        with mc.Integrator(terms=w.terms, per_orbit=force, **kw) as I:
+            g = I.integrate(w.states, 1.0, 1000, 3, shadow_eps=1e-8)
+            info = I.launch_info()
+        assert info["local_bytes"] == 0
+        assert (info["variant"] & 7) == (6 if force is None else 3)           # QM + (kappa-only | per-orbit)
+        assert info["blocks_per_sm"] == (3 if force is None else 2)
+        assert np.array_equal(g.status.cpu().numpy(), o.status)
+        assert rel_state_err(g.states.cpu().numpy()[:, ok], o.states[:, ok]) <= STATE_RTOL
+        assert np.abs(g.fli.cpu().numpy()[ok] - o.fli[ok]).max() < 1e-3
+        assert drift(g.states.cpu().numpy()[:, ok], o.invariants[0:6][:, ok], **w.subset(np.where(ok)[0]).params()) <= DRIFT_TOL
+        got[force] = g.states.cpu().numpy()
+    assert rel_state_err(got[None][:, ok], got[1][:, ok]) <= STATE_RTOL
+    off = workloads.config3(n_r=12, n_theta=13, qm=False)
+    with mc.Integrator(terms=off.terms, **kw) as I:
+        g = I.integrate(off.states, 1.0, 300, 3, shadow_eps=1e-8)
+        assert (I.launch_info()["variant"] & 7) == 0                           # uniform kernel: kappa does not enter
+    oo = oracle.integrate(off.states, 1.0, 300, 3, shadow_eps=1e-8, **off.params())
+    live = oo.status == 0
+    assert rel_state_err(g.states.cpu().numpy()[:, live], oo.states[:, live]) <= STATE_RTOL
+
+
 def test_mode2_dual_scaling_parity_on_unskipped_orbits(mc):
     w = workloads.config0(128)
     with mc.Integrator(newton_iters=4) as I:
@@ -407,7 +447,7 @@ def _all_outputs(I, z, n_steps, mode, eps):
     return [t.cpu().numpy() for t in outs], I.launch_info()
 
 
-@pytest.mark.parametrize("case", ["uniform-shadow", "per-orbit-shadow", "dropped-cells", "mode2-no-shadow"])
+@pytest.mark.parametrize("case", ["uniform-shadow", "per-orbit-shadow", "kappa-shadow", "dropped-cells", "mode2-no-shadow"])
 def test_chunked_scheduling_never_changes_a_bit(mc, case):
     """the kernel's work items are chunks of steps whose state rests in a carry buffer
     between chunks.  Any chunk length -- a divisor of the run, one that cuts renormalisation intervals, a single
@@ -415,9 +455,10 @@ def test_chunked_scheduling_never_changes_a_bit(mc, case):
     mode, eps, kw = 3, 1e-8, {}
     if case == "uniform-shadow":
         z = workloads.config0(300).states
-    elif case == "per-orbit-shadow":
+    elif case in ("per-orbit-shadow", "kappa-shadow"):
         w = workloads.config3(n_r=9, n_theta=23, qm=True)
-        z, kw = w.states, dict(terms=w.terms, **{k: v for k, v in w.params().items() if k != "terms"})
+        z, kw = w.states, dict(terms=w.terms, per_orbit=(1 if case == "per-orbit-shadow" else None),
+                               **{k: v for k, v in w.params().items() if k != "terms"})
     elif case == "dropped-cells":
         z = workloads.scan_grid(12, 11, r_lo=6.0, r_hi=16.0)[0]
     else:
@@ -579,7 +620,7 @@ def test_checkpoint_resume_is_bitwise_identical_to_one_run(mc, case):
         z = workloads.config0(300).states
     elif case == "per-orbit-qm-rk5":
         w = workloads.config3(n_r=7, n_theta=19, qm=True)
-        z, kw = w.states, dict(terms=w.terms, integrator=mc.MC_INTEG_RK5, **{k: v for k, v in w.params().items() if k != "terms"})
+        z, kw = w.states, dict(terms=w.terms, integrator=mc.MC_INTEG_RK5, per_orbit=1, **{k: v for k, v in w.params().items() if k != "terms"})
     elif case == "dropped-cells":
         z = workloads.scan_grid(12, 11, r_lo=6.0, r_hi=16.0)[0]
     else:
@@ -656,7 +697,7 @@ def test_config3_full_size_quadrupole_sampled_against_oracle(mc):
     with mc.Integrator(terms=w.terms, **kw) as I:
         g = I.integrate(w.states, w.h, w.n_steps, 3, shadow_eps=w.shadow_eps)
         info = I.launch_info()
-    assert info["local_bytes"] == 0 and info["variant"] & 3 == 3
+    assert info["local_bytes"] == 0 and info["variant"] & 7 == 6          # QM on, per-orbit kappa only (per_orbit = 2)
     gs, gz, gfli = g.status.cpu().numpy(), g.states.cpu().numpy(), g.fli.cpu().numpy()
     live = gs == 0
     assert 0.7 < live.mean() < 1.0

@@ -17,7 +17,7 @@ from . import build as _build
 LONG_DOUBLE = 0
 DOUBLE = 1
 
-TERM_1PN, TERM_2PN, TERM_SO, TERM_S1S2, TERM_QM = 1, 2, 4, 8, 16
+TERM_1PN, TERM_2PN, TERM_SO, TERM_S1S2, TERM_QM, TERM_RR = 1, 2, 4, 8, 16, 32
 TERMS_DEFAULT = TERM_1PN | TERM_2PN | TERM_SO | TERM_S1S2
 
 _lib = None
@@ -52,12 +52,13 @@ def _params(n, beta, chi1, chi2, kq1, kq2):
     return [_par(v, n) for v in (beta, chi1, chi2, kq1, kq2)]
 
 
-_WHAT = {"H": (0, 1), "J": (1, 3), "rhs": (2, 12), "gradient": (3, 12), "integrals": (4, 6)}
+_WHAT = {"H": (0, 1), "J": (1, 3), "rhs": (2, 12), "gradient": (3, 12), "integrals": (4, 6), "rhs16": (5, 16)}
 
 
 def evaluate(what, z, beta=1.0, chi1=1.0, chi2=1.0, kq1=1.0, kq2=1.0, terms=TERMS_DEFAULT,
              precision=LONG_DOUBLE):
-    """what in {"H","J","rhs","gradient","integrals"}; returns array of shape (rows, n)."""
+    """what in {"H","J","rhs","gradient","integrals","rhs16"}; returns array of shape (rows, n).
+    rhs16 = rhs plus the rates of the dissipation integrals (dW/dt, dG/dt; zero without TERM_RR)."""
     z = _states(z)
     n = z.shape[1]
     code, rows = _WHAT[what]
@@ -149,6 +150,7 @@ class Result:
     steps_done: np.ndarray   # (n,) int64
     gn_steps: np.ndarray     # (n,) int64: Gauss-Newton steps of mode 3 over accepted steps, orbit + shadow
     samples: np.ndarray = None   # (n_steps // sample_interval, 12, n): orbit states after steps interval, 2 interval, ...
+    diss: np.ndarray = None      # (4, n): W, Gx, Gy, Gz, the work and torque integrals of the 2.5PN force (zero without TERM_RR)
     shadow: np.ndarray = None    # (16, n) with want_shadow: the shadow's final state (12 rows), then E0', J0' it is corrected onto
 
 
@@ -166,6 +168,7 @@ def integrate(z, h, n_steps, mode, shadow_eps=0.0, beta=1.0, chi1=1.0, chi2=1.0,
         res.samples = np.empty((n_steps // sample_interval, 12, n))
     if want_shadow:
         res.shadow = np.empty((16, n))
+    res.diss = np.empty((4, n))
     lib().oracle_integrate(ctypes.c_int(precision), ctypes.c_int64(n), _p(z), *[_p(a) for a in pa],
                            ctypes.c_uint32(terms), ctypes.c_double(h), ctypes.c_int64(n_steps),
                            ctypes.c_int(mode), ctypes.c_double(shadow_eps), ctypes.c_int(renorm_interval),
@@ -173,7 +176,7 @@ def integrate(z, h, n_steps, mode, shadow_eps=0.0, beta=1.0, chi1=1.0, chi2=1.0,
                            ctypes.c_double(r_merge), ctypes.c_double(r_escape), _p(res.states),
                            _p(res.invariants), _p(res.fli), _p(res.status), _p(res.steps_done),
                            _p(res.gn_steps), ctypes.c_int(n_threads), ctypes.c_int(integrator),
-                           ctypes.c_int64(sample_interval), _p(res.samples), _p(res.shadow))
+                           ctypes.c_int64(sample_interval), _p(res.samples), _p(res.shadow), _p(res.diss))
     return res
 
 

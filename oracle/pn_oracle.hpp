@@ -48,17 +48,25 @@ template <class T> inline V3<T> cross(V3<T> a, V3<T> b) {
 }
 
 // State of one trajectory: z = (r, p, S1hat, S2hat).
-template <class T> struct State { V3<T> r, p, s1, s2; };
+// Diss: with the 2.5PN radiation reaction (TERM_RR) the integrator also carries the work W = int (dr/dt).F dt and the
+// torque integral G = int r x F dt of the dissipative force (the "integral invariant relation" of PAPER.md:221:
+// H(t) - W(t) and J(t) - G(t) stay constant along the exact flow).  They are integrated by the same RK scheme as
+// extra components; without TERM_RR their derivatives are zero and they never touch z.
+template <class T> struct Diss { T w; V3<T> g; };
+template <class T> struct State { V3<T> r, p, s1, s2; Diss<T> d; };
+template <class T> inline Diss<T> operator+(Diss<T> a, Diss<T> b) { return {a.w + b.w, a.g + b.g}; }
+template <class T> inline Diss<T> operator-(Diss<T> a, Diss<T> b) { return {a.w - b.w, a.g - b.g}; }
+template <class T> inline Diss<T> operator*(T s, Diss<T> a) { return {s * a.w, s * a.g}; }
 template <class T> inline State<T> operator+(State<T> a, State<T> b) {
-  return {a.r + b.r, a.p + b.p, a.s1 + b.s1, a.s2 + b.s2};
+  return {a.r + b.r, a.p + b.p, a.s1 + b.s1, a.s2 + b.s2, a.d + b.d};
 }
 template <class T> inline State<T> operator-(State<T> a, State<T> b) {
-  return {a.r - b.r, a.p - b.p, a.s1 - b.s1, a.s2 - b.s2};
+  return {a.r - b.r, a.p - b.p, a.s1 - b.s1, a.s2 - b.s2, a.d - b.d};
 }
-template <class T> inline State<T> operator*(T s, State<T> a) { return {s * a.r, s * a.p, s * a.s1, s * a.s2}; }
+template <class T> inline State<T> operator*(T s, State<T> a) { return {s * a.r, s * a.p, s * a.s1, s * a.s2, s * a.d}; }
 template <class T> inline T norm12sq(State<T> a) { return dot(a.r, a.r) + dot(a.p, a.p) + dot(a.s1, a.s1) + dot(a.s2, a.s2); }
 
-enum : uint32_t { TERM_1PN = 1u, TERM_2PN = 2u, TERM_SO = 4u, TERM_S1S2 = 8u, TERM_QM = 16u };
+enum : uint32_t { TERM_1PN = 1u, TERM_2PN = 2u, TERM_SO = 4u, TERM_S1S2 = 8u, TERM_QM = 16u, TERM_RR = 32u };
 
 // Dynamic parameters of one binary (kq = quadrupole
 // coefficient of DESIGN.md reading R16, kq = 1 for black holes).
@@ -198,13 +206,43 @@ template <class T> Grad<T> gradient(const State<T>& z, const Params<T>& P) {
   return g;
 }
 
-// Equations of motion, eqs (6)-(7) without a_2.5PN:
-// dr/dt = dH/dp, dp/dt = -dH/dr, dS_i/dt = Omega_i x S_i, Omega_i = dH/dS_i.
+// 2.5PN radiation reaction, the a_2.5PN of eq (6) ("the acceleration from the H_2.5PN radiation
+// reaction in ADM coordinates").  PAPER.md does not print it (it points to Levin et al. 2011); DESIGN.md reading
+// R21 takes the leading-order radiation-reaction acceleration in its general two-parameter gauge form (Iyer & Will
+// 1993, 1995), per unit reduced mass and with v = p at this order,
+//   a_RR = (8/5) eta / r^3 * { (n.p) n [a1 p^2 + a2 / r + a3 (n.p)^2] - p [b1 p^2 + b2 / r + b3 (n.p)^2] },
+//   a1 = 3 + 3 B, a2 = 23/3 + 2 A - 3 B, a3 = -5 B, b1 = 2 + A, b2 = 2 - A, b3 = -3 - 3 A,
+// in the ADM gauge of Schaefer (1985), (A, B) = (5/3, 3): a = (12, 2, -15), b = (11/3, 1/3, -8).
+// Every gauge gives the same orbit-averaged energy and angular momentum fluxes (Peters & Mathews 1963, Peters 1964),
+// which is what the pins check; the gauge itself is a reading.
+template <class T> V3<T> rr_force(const State<T>& z, const Params<T>& P) {
+  const T A = T(5) / T(3), B = T(3);
+  const T a1 = T(3) + T(3) * B, a2 = T(23) / T(3) + T(2) * A - T(3) * B, a3 = T(0) - T(5) * B;
+  const T b1 = T(2) + A, b2 = T(2) - A, b3 = T(0) - T(3) - T(3) * A;
+  const T r = o_sqrt(dot(z.r, z.r));
+  const V3<T> n = (T(1) / r) * z.r;
+  const T p2 = dot(z.p, z.p);
+  const T np = dot(n, z.p);
+  const T ca = a1 * p2 + a2 / r + a3 * np * np;
+  const T cb = b1 * p2 + b2 / r + b3 * np * np;
+  return (T(8) * P.eta() / (T(5) * r * r * r)) * ((np * ca) * n - cb * z.p);
+}
+
+// Equations of motion, eqs (6)-(7):
+// dr/dt = dH/dp, dp/dt = -dH/dr (+ a_2.5PN with TERM_RR), dS_i/dt = Omega_i x S_i, Omega_i = dH/dS_i.
 // |S_i| is a parameter, so dS_i_hat/dt = Omega_i x S_i_hat.
+// With TERM_RR also dW/dt = (dr/dt).a_2.5PN and dG/dt = r x a_2.5PN (see Diss).
 template <class T> State<T> rhs(const State<T>& z, const Params<T>& P) {
   const Grad<T> g = gradient(z, P);
   const V3<T> zero = {T(0), T(0), T(0)};
-  return {g.dHdp, zero - g.dHdr, cross(g.dHdS1, z.s1), cross(g.dHdS2, z.s2)};
+  State<T> f = {g.dHdp, zero - g.dHdr, cross(g.dHdS1, z.s1), cross(g.dHdS2, z.s2), {T(0), zero}};
+  if (P.terms & TERM_RR) {
+    const V3<T> F = rr_force(z, P);
+    f.p = f.p + F;
+    f.d.w = dot(g.dHdp, F);
+    f.d.g = cross(z.r, F);
+  }
+  return f;
 }
 
 // Classical RK4 (c = 0, 1/2, 1/2, 1; b = 1/6, 1/3, 1/3, 1/6); R9.
@@ -430,6 +468,12 @@ OrbitResult<T> integrate_orbit(State<T> z, const Params<T>& P, T h, int64_t n_st
                                int64_t sample_interval, Sampler sampler) {
   OrbitResult<T> out;
   const bool shadow = !(shadow_eps == T(0));
+  const bool rr = (P.terms & TERM_RR) != 0;
+  const V3<T> zero3 = {T(0), T(0), T(0)};
+  z.d = {T(0), zero3};
+  // With radiation reaction the manifold moves: the correction targets E0 + W, J0 + G (integral invariant relation,
+  // PAPER.md:221), W and G being the dissipation integrals the step itself has just advanced.
+  auto moved = [&](const Refs<T>& R0, const State<T>& zz) { return rr ? Refs<T>{R0.E0 + zz.d.w, R0.J0 + zz.d.g} : R0; };
   if (O.mode >= 1) { z.s1 = unit(z.s1); z.s2 = unit(z.s2); }
   Refs<T> R = references(z, P);
   six_integrals(z, P, out.inv0);
@@ -446,11 +490,11 @@ OrbitResult<T> integrate_orbit(State<T> z, const Params<T>& P, T h, int64_t n_st
   while (k < n_steps) {
     int gn = 0, gns = 0;
     State<T> zn = base_step(z, h, P, O.integrator);
-    if (!correct(zn, P, R, O.mode, O.newton_iters, T(O.newton_tol), &gn)) flag = ST_NEWTON_FLAG;
+    if (!correct(zn, P, moved(R, zn), O.mode, O.newton_iters, T(O.newton_tol), &gn)) flag = ST_NEWTON_FLAG;
     State<T> zsn = zs;
     if (shadow) {
       zsn = base_step(zs, h, P, O.integrator);
-      correct(zsn, P, Rs, O.mode, O.newton_iters, T(O.newton_tol), &gns);
+      correct(zsn, P, moved(Rs, zsn), O.mode, O.newton_iters, T(O.newton_tol), &gns);
     }
     // status check on the completed step (R13); on failure keep the last good state
     if (!finite_state(zn) || !finite_state(zsn)) { status = ST_NONFINITE; break; }
@@ -467,6 +511,7 @@ OrbitResult<T> integrate_orbit(State<T> z, const Params<T>& P, T h, int64_t n_st
       zs = z + (d0 / d) * dz;
       if (O.mode >= 1) { zs.s1 = unit(zs.s1); zs.s2 = unit(zs.s2); }
       Rs = references(zs, P);  // DESIGN.md R11
+      zs.d = {T(0), zero3};    // its dissipation integrals restart with its references
     }
   }
   if (sample_interval > 0)   // a dropped orbit keeps reporting its frozen state

@@ -42,7 +42,12 @@ inline double to_double(double x) { return x; }
 
 template <class T> State<T> load_state(const double* s, int64_t n, int64_t i) {
   auto g = [&](int c) { return T(s[(int64_t)c * n + i]); };
-  return {{g(0), g(1), g(2)}, {g(3), g(4), g(5)}, {g(6), g(7), g(8)}, {g(9), g(10), g(11)}};
+  return {{g(0), g(1), g(2)}, {g(3), g(4), g(5)}, {g(6), g(7), g(8)}, {g(9), g(10), g(11)}, {T(0.0), {T(0.0), T(0.0), T(0.0)}}};
+}
+// rows 12-15 of a [16][n] array: W, Gx, Gy, Gz (the dissipation integrals / their time derivatives)
+template <class T> void store_diss(double* s, int64_t n, int64_t i, const Diss<T>& d) {
+  const T v[4] = {d.w, d.g.x, d.g.y, d.g.z};
+  for (int c = 0; c < 4; ++c) s[(int64_t)(12 + c) * n + i] = to_double(v[c]);
 }
 template <class T> void store_state(double* s, int64_t n, int64_t i, const State<T>& z) {
   const T v[12] = {z.r.x, z.r.y, z.r.z, z.p.x, z.p.y, z.p.z, z.s1.x, z.s1.y, z.s1.z, z.s2.x, z.s2.y, z.s2.z};
@@ -57,7 +62,7 @@ Params<T> load_params(const double* beta, const double* chi1, const double* chi2
 struct ParamArrays { const double *beta, *chi1, *chi2, *kq1, *kq2; uint32_t terms; };
 
 // what: 0 H -> out[1][n]; 1 J -> out[3][n]; 2 rhs -> out[12][n];
-// 3 gradient (dH/dr, dH/dp, dH/dS1, dH/dS2) -> out[12][n]; 4 six integrals -> out[6][n]
+// 3 gradient (dH/dr, dH/dp, dH/dS1, dH/dS2) -> out[12][n]; 4 six integrals -> out[6][n]; 5 rhs + (dW/dt, dG/dt) -> out[16][n]
 template <class T> void eval_t(int what, int64_t n, const double* states, const ParamArrays& A, double* out) {
   for (int64_t i = 0; i < n; ++i) {
     const State<T> z = load_state<T>(states, n, i);
@@ -71,7 +76,11 @@ template <class T> void eval_t(int what, int64_t n, const double* states, const 
       store_state(out, n, i, rhs(z, P));
     } else if (what == 3) {
       const Grad<T> g = gradient(z, P);
-      store_state(out, n, i, State<T>{g.dHdr, g.dHdp, g.dHdS1, g.dHdS2});
+      store_state(out, n, i, State<T>{g.dHdr, g.dHdp, g.dHdS1, g.dHdS2, z.d});
+    } else if (what == 5) {   // rhs with the dissipation rates: out[16][n], rows 12-15 = dW/dt, dG/dt
+      const State<T> f = rhs(z, P);
+      store_state(out, n, i, f);
+      store_diss(out, n, i, f.d);
     } else {
       T v[6];
       six_integrals(z, P, v);
@@ -104,7 +113,7 @@ template <class T>
 void integrate_t(int64_t n, const double* states, const ParamArrays& A, double h, int64_t n_steps,
                  double shadow_eps, const Options& O, double* out_states, double* out_inv, double* out_fli,
                  int32_t* out_status, int64_t* out_step, int64_t* out_gn, int n_threads,
-                 int64_t sample_interval, double* out_samples, double* out_shadow) {
+                 int64_t sample_interval, double* out_samples, double* out_shadow, double* out_diss) {
 #pragma omp parallel for schedule(static) num_threads(n_threads)
   for (int64_t i = 0; i < n; ++i) {
     const State<T> z = load_state<T>(states, n, i);
@@ -123,6 +132,10 @@ void integrate_t(int64_t n, const double* states, const ParamArrays& A, double h
     if (out_status) out_status[i] = R.status;
     if (out_step) out_step[i] = R.steps_done;
     if (out_gn) out_gn[i] = R.gn_steps;
+    if (out_diss) {     // [4][n]: W, Gx, Gy, Gz of the orbit at the end of the run
+      const T v[4] = {R.z.d.w, R.z.d.g.x, R.z.d.g.y, R.z.d.g.z};
+      for (int c = 0; c < 4; ++c) out_diss[(int64_t)c * n + i] = to_double(v[c]);
+    }
     if (out_shadow) {   // [16][n]: the shadow's final state, then E0', J0' (the integrals it is corrected onto)
       store_state(out_shadow, n, i, R.zs);
       const T refs[4] = {R.Es0, R.Js0.x, R.Js0.y, R.Js0.z};
@@ -179,16 +192,16 @@ int oracle_integrate(int precision, int64_t n, const double* states, const doubl
                      double newton_tol, double r_merge, double r_escape, double* out_states,
                      double* out_invariants, double* out_fli, int32_t* out_status, int64_t* out_step,
                      int64_t* out_gn_steps, int n_threads, int integrator, int64_t sample_interval,
-                     double* out_samples, double* out_shadow) {
+                     double* out_samples, double* out_shadow, double* out_diss) {
   const ParamArrays A = {beta, chi1, chi2, kq1, kq2, terms};
   const Options O = {mode, renorm_interval, newton_iters, newton_tol, r_merge, r_escape, integrator};
   if (n_threads <= 0) n_threads = omp_get_max_threads();
   if (precision == 0)
     integrate_t<long double>(n, states, A, h, n_steps, shadow_eps, O, out_states, out_invariants, out_fli,
-                             out_status, out_step, out_gn_steps, n_threads, sample_interval, out_samples, out_shadow);
+                             out_status, out_step, out_gn_steps, n_threads, sample_interval, out_samples, out_shadow, out_diss);
   else
     integrate_t<double>(n, states, A, h, n_steps, shadow_eps, O, out_states, out_invariants, out_fli,
-                        out_status, out_step, out_gn_steps, n_threads, sample_interval, out_samples, out_shadow);
+                        out_status, out_step, out_gn_steps, n_threads, sample_interval, out_samples, out_shadow, out_diss);
   return 0;
 }
 

@@ -37,7 +37,15 @@ enum mc_terms {
   MC_TERM_2PN = 2u,   /* H_2PN                                            */
   MC_TERM_SO = 4u,    /* spin-orbit, L-terms of eqs (8)-(9) */
   MC_TERM_S1S2 = 8u,  /* eq (3)                              */
-  MC_TERM_QM = 16u    /* eqs (4)-(5), quadrupole-monopole */
+  MC_TERM_QM = 16u,   /* eqs (4)-(5), quadrupole-monopole */
+  MC_TERM_RR = 32u    /* a_2.5PN of eq (6): leading-order radiation reaction in the ADM gauge
+                         (R21; not printed in the paper).  NON-conservative: every trajectory also
+                         carries the work W = int (dr/dt).a dt and the torque integral G = int r x a dt of the
+                         force, and the correction (modes 2, 3) targets E0 + W and J0 + G, the "integral invariant
+                         relation" of PAPER.md:221; see mc_get_dissipation.  Default off.  One combination is not
+                         built: per_orbit = 1 together with MC_INTEG_RK5 (mc_integrate returns MC_EINVAL; the 37
+                         per-orbit constants, six stages and 16 components exceed the 255-register budget and the
+                         library ships no kernel that spills)                                               */
 };
 
 /* Correction applied after every RK4 step. */
@@ -173,6 +181,14 @@ int mc_integrate_host(mc_handle* h, const double* states, int64_t n_orbits, doub
  * number of completed steps.  Either pointer may be NULL. */
 int mc_get_status(mc_handle* h, int32_t* out_status, int64_t* out_step);
 
+/* Moving reference integrals of the most recent mc_integrate on a handle created with MC_TERM_RR, copied (stream-
+ * ordered) into out_wg, DEVICE double[4][n_orbits]: E0 + W, J0x + Gx, J0y + Gy, J0z + Gz of every orbit at the end of
+ * the run, W and G being the work and torque integrals of the radiation-reaction force (H(t) - W(t) and
+ * J(t) - G(t) are constant along the exact flow, so rows 6-9 of out_invariants equal these to truncation error
+ * without correction and to round-off with it; W = row 0 of this minus row 0 of out_invariants).  MC_EINVAL without
+ * MC_TERM_RR. */
+int mc_get_dissipation(mc_handle* h, double* out_wg);
+
 /* Work done by the most recent mc_integrate on this handle: out_gn_steps, DEVICE int64[n_orbits] = number
  * of Gauss-Newton steps correction mode 3 took over all accepted steps of the orbit and its shadow
  * (0 for the other modes).  Stream-ordered copy.  bench.py derives the algorithmic flop count from it. */
@@ -181,9 +197,11 @@ int mc_get_work(mc_handle* h, int64_t* out_gn_steps);
 /* Evaluate pieces of the model on the device with the handle's parameters (used by the parity tests
  * to compare the kernel's fused routines with the oracle one by one).  states: DEVICE double[12][n].
  *   what = 0: out[1][n]  = H                     (eq 1)
- *   what = 1: out[12][n] = dz/dt                 (eqs 6-9: dH/dp, -dH/dr, Omega_i x S_i_hat)
+ *   what = 1: out[12][n] = dz/dt                 (eqs 6-9: dH/dp, -dH/dr, Omega_i x S_i_hat); with MC_TERM_RR
+ *             out[16][n], rows 12-15 = dW/dt, dG/dt
  *   what = 2: out[6][n]  = E, Jx, Jy, Jz, |S1hat|, |S2hat|
- *   what = 3: out[12][n] = one step of the base integrator (params.integrator) of size step_h, no correction
+ *   what = 3: out[12][n] = one step of the base integrator (params.integrator) of size step_h, no correction;
+ *             with MC_TERM_RR out[16][n], rows 12-15 = W, G accumulated over the step (from zero)
  *   what = 4: out[12][n] = correction operator of mode `mode` applied to states, with references
  *             refs = DEVICE double[4][n] (E0, J0x, J0y, J0z); required for every mode (MC_EINVAL if NULL)
  * Asynchronous on the handle's stream. */
@@ -198,7 +216,7 @@ typedef struct mc_launch_info {
   int32_t blocks_per_sm;        /* occupancy API result for that block size       */
   int32_t num_sms;
   int32_t smem_bytes;           /* dynamic shared memory per block                */
-  int32_t variant;              /* bit0 per-orbit params, bit1 QM, bit2 per-orbit kq only, bits 4-5 mode, bit 8 RK5 */
+  int32_t variant;              /* bit0 per-orbit params, bit1 QM, bit2 per-orbit kq only, bit3 2.5PN, bits 4-5 mode, bit 8 RK5 */
   int64_t trajectories;         /* threads doing work = n_orbits * (1 + shadow)   */
   int32_t chunk_steps;          /* steps per work item                             */
   int32_t n_chunks;             /* work items per 32-trajectory unit              */
@@ -225,6 +243,8 @@ int mc_fp64_peak(int32_t device, double millis, double* out_tflops, double* out_
  *   references     E0, J0 of a state (H + J)
  *   renorm         one shadow renormalisation (distance, pull-back, eq 10, re-referenced integrals)
  * A trajectory-step costs base_step + correct_fixed + status + gn_step x (Gauss-Newton steps taken, mc_get_work).
+ * With MC_TERM_RR the RHS, the base step and the renormalisation include the radiation-reaction force and the four
+ * dissipation integrals (16 components per trajectory).
  * Errors: MC_EINVAL (null, unknown term bit / mode / integrator, newton_iters outside 1..16). */
 typedef struct mc_op_counts { int64_t fma, mul, add, special; } mc_op_counts;
 typedef struct mc_flop_model_t {

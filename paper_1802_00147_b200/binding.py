@@ -11,13 +11,13 @@ from typing import Optional
 
 from . import build as _build
 
-MC_TERM_1PN, MC_TERM_2PN, MC_TERM_SO, MC_TERM_S1S2, MC_TERM_QM = 1, 2, 4, 8, 16
+MC_TERM_1PN, MC_TERM_2PN, MC_TERM_SO, MC_TERM_S1S2, MC_TERM_QM, MC_TERM_RR = 1, 2, 4, 8, 16, 32
 TERMS_DEFAULT = MC_TERM_1PN | MC_TERM_2PN | MC_TERM_SO | MC_TERM_S1S2
 MC_OK, MC_EINVAL, MC_ECUDA, MC_EARCH, MC_ENOMEM = 0, -1, -2, -3, -4
 MC_INTEG_RK4, MC_INTEG_RK5 = 0, 1
 
 # every symbol include/mc.h declares (tests/test_abi.py checks the header against this list)
-EXPORTS = ["mc_params_default", "mc_create", "mc_integrate", "mc_integrate_sampled", "mc_integrate_ex", "mc_carry_bytes", "mc_integrate_host", "mc_get_status", "mc_get_work", "mc_eval",
+EXPORTS = ["mc_params_default", "mc_create", "mc_integrate", "mc_integrate_sampled", "mc_integrate_ex", "mc_carry_bytes", "mc_integrate_host", "mc_get_status", "mc_get_work", "mc_get_dissipation", "mc_eval",
            "mc_last_launch_info", "mc_fp64_peak", "mc_flop_model", "mc_destroy", "mc_strerror"]
 
 
@@ -94,6 +94,7 @@ def load_library():
     lib.mc_integrate_host.argtypes = [vp, vp, i64, dbl, i64, i32, dbl, vp, vp, vp, vp, vp]
     lib.mc_get_status.argtypes = [vp, vp, vp]
     lib.mc_get_work.argtypes = [vp, vp]
+    lib.mc_get_dissipation.argtypes = [vp, vp]
     lib.mc_eval.argtypes = [vp, i32, vp, i64, dbl, i32, vp, vp]
     lib.mc_last_launch_info.argtypes = [vp, ctypes.POINTER(mc_launch_info)]
     lib.mc_fp64_peak.argtypes = [i32, dbl, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
@@ -308,6 +309,8 @@ class Integrator:
         z = self._dev(states)
         n = z.shape[1]
         code, rows = self._WHAT[what]
+        if (self.params.terms & MC_TERM_RR) and what in ("rhs", "rk4_step"):
+            rows = 16                                   # + the dissipation integrals / their rates (include/mc.h)
         out = torch.empty((rows, n), dtype=torch.float64, device=self.device)
         r = self._dev(refs) if refs is not None else None
         _check(self._lib.mc_eval(self._h, code, z.data_ptr(), n, float(h), int(mode),
@@ -319,6 +322,14 @@ class Integrator:
         torch = self._torch
         out = torch.empty(n, dtype=torch.int64, device=self.device)
         _check(self._lib.mc_get_work(self._h, out.data_ptr()))
+        return out
+
+    def dissipation(self, n):
+        """mc_get_dissipation: the moving references E0 + W, J0 + G per orbit at the end of the last integrate (handle
+        created with MC_TERM_RR) -> (4, n); subtract rows 0-3 of the invariants to get W, G."""
+        torch = self._torch
+        out = torch.empty((4, n), dtype=torch.float64, device=self.device)
+        _check(self._lib.mc_get_dissipation(self._h, out.data_ptr()))
         return out
 
     def launch_info(self) -> dict:

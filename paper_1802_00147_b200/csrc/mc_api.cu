@@ -54,7 +54,7 @@ struct mc_handle {
   cudaStream_t stream;
   int num_sms;
   int64_t last_n;            // orbits of the last mc_integrate (status buffers valid for these)
-  DeviceBuf status, step, gn;   // int32[n], int64[n], int64[n]
+  DeviceBuf status, step, gn, diss;   // int32[n], int64[n], int64[n], double[4][n] (MC_TERM_RR)
   DeviceBuf sched, carry_d, carry_i, carry_g;   // work queue + per-unit flags; carried state between chunks
   DeviceBuf h_in, h_out, h_inv, h_fli;   // scratch of mc_integrate_host
   mc_launch_info info;
@@ -80,21 +80,28 @@ eval_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ mc::Int
   const int64_t o = active ? t : A.n - 1;
   using CP = typename mc::ConstsOf<PARAMS>::type;
   const CP c = mc::make_consts<PARAMS, CP>(uc, A, o, smem);
-  double z[12], f[12];
+  double z[16], f[16];
 #pragma unroll
   for (int i = 0; i < 12; ++i) z[i] = A.states[(int64_t)i * A.n + o];
+  z[12] = z[13] = z[14] = z[15] = 0.0;
   int rows = 12;
+  const bool rr = (A.terms & MC_TERM_RR) != 0;
   if (what == 0) {
     f[0] = mc::hamiltonian<QM>(c, z);
     rows = 1;
   } else if (what == 1) {
-    mc::pn_rhs<QM>(c, z, f);
+    if (rr) { mc::pn_rhs<QM, true>(c, z, f); rows = 16; }
+    else mc::pn_rhs<QM, false>(c, z, f);
   } else if (what == 2) {
     mc::six_integrals<QM>(c, z, f);
     rows = 6;
   } else if (what == 3) {
-    if (A.integrator == 1) mc::rk5_step<QM>(c, z, A.h, f);
-    else mc::rk4_step<QM>(c, z, A.h, f);
+    if (rr) {
+      if (A.integrator == 1) mc::rk5_step<QM, true>(c, z, A.h, f);
+      else mc::rk4_step<QM, true>(c, z, A.h, f);
+      rows = 16;
+    } else if (A.integrator == 1) mc::rk5_step<QM, false>(c, z, A.h, f);
+    else mc::rk4_step<QM, false>(c, z, A.h, f);
   } else {
     mc::Refs R;
     R.E0 = refs[o];
@@ -108,7 +115,7 @@ eval_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ mc::Int
   }
   if (active) {
 #pragma unroll
-    for (int i = 0; i < 12; ++i)
+    for (int i = 0; i < 16; ++i)
       if (i < rows) out[(int64_t)i * A.n + o] = f[i];
   }
 }
@@ -174,7 +181,7 @@ int mc_params_default(mc_params* p) {
 int mc_create(const mc_params* params, mc_handle** out_handle) {
   if (!params || !out_handle) return MC_EINVAL;
   if (params->struct_size != sizeof(mc_params)) return MC_EINVAL;
-  if (params->terms & ~31u) return MC_EINVAL;
+  if (params->terms & ~63u) return MC_EINVAL;
   if (params->renorm_interval <= 0 || params->newton_iters < 1 || params->newton_iters > 16) return MC_EINVAL;
   if (params->chunk_steps < 0) return MC_EINVAL;
   if (params->integrator != MC_INTEG_RK4 && params->integrator != MC_INTEG_RK5) return MC_EINVAL;
@@ -262,11 +269,14 @@ static int integrate_impl(mc_handle* h, const double* states, int64_t n_orbits, 
   if (rc) return rc;
   rc = h->gn.reserve(sizeof(int64_t) * (size_t)n_orbits);
   if (rc) return rc;
+  const bool rr = (h->P.terms & MC_TERM_RR) != 0;
+  if (rr && (rc = h->diss.reserve(sizeof(double) * 4 * (size_t)n_orbits))) return rc;
 
   mc::IntegrateArgs A;
   fill_args(h, A);
   A.states = states; A.out_states = out_states; A.out_inv = out_invariants; A.out_fli = shadow ? out_fli : nullptr;
   A.out_status = (int32_t*)h->status.p; A.out_step = (int64_t*)h->step.p; A.out_gn = (int64_t*)h->gn.p;
+  A.out_diss = rr ? (double*)h->diss.p : nullptr;
   A.n = n_orbits; A.n_steps = n_steps; A.h = step_h; A.shadow_eps = shadow_eps;
   A.samples = sample_interval > 0 ? out_samples : nullptr;
   A.sample_interval = sample_interval > 0 ? (int32_t)sample_interval : 1;
@@ -274,11 +284,12 @@ static int integrate_impl(mc_handle* h, const double* states, int64_t n_orbits, 
   const bool qm = (h->P.terms & MC_TERM_QM) != 0;
   mc::LaunchFn fn = nullptr;
   switch (correction_mode) {
-    case 0: fn = mc::launcher_mode0(h->P.per_orbit, qm, h->P.integrator); break;
-    case 1: fn = mc::launcher_mode1(h->P.per_orbit, qm, h->P.integrator); break;
-    case 2: fn = mc::launcher_mode2(h->P.per_orbit, qm, h->P.integrator); break;
-    default: fn = mc::launcher_mode3(h->P.per_orbit, qm, h->P.integrator); break;
+    case 0: fn = mc::launcher_mode0(h->P.per_orbit, qm, h->P.integrator, rr); break;
+    case 1: fn = mc::launcher_mode1(h->P.per_orbit, qm, h->P.integrator, rr); break;
+    case 2: fn = mc::launcher_mode2(h->P.per_orbit, qm, h->P.integrator, rr); break;
+    default: fn = mc::launcher_mode3(h->P.per_orbit, qm, h->P.integrator, rr); break;
   }
+  if (!fn) return MC_EINVAL;   // per_orbit = 1 with RK5 and MC_TERM_RR: not built (register budget; include/mc.h)
   const int64_t traj = n_orbits * (shadow ? 2 : 1);
   A.n_units = (traj + 31) / 32;
   if (A.n_units > 0x3fffffffLL) return MC_EINVAL;
@@ -333,7 +344,7 @@ static int integrate_impl(mc_handle* h, const double* states, int64_t n_orbits, 
   h->info.num_sms = h->num_sms;
   h->info.smem_bytes = (int32_t)ki.smem;
   const int kparams = (h->P.per_orbit == 2 && !qm) ? 0 : h->P.per_orbit;   // kappa is unused without the QM term
-  h->info.variant = (kparams == 1 ? 1 : 0) | (qm ? 2 : 0) | (kparams == 2 ? 4 : 0) | (correction_mode << 4) | (h->P.integrator << 8);
+  h->info.variant = (kparams == 1 ? 1 : 0) | (qm ? 2 : 0) | (kparams == 2 ? 4 : 0) | (rr ? 8 : 0) | (correction_mode << 4) | (h->P.integrator << 8);
   h->info.trajectories = traj;
   return MC_OK;
 }
@@ -354,6 +365,15 @@ int mc_get_work(mc_handle* h, int64_t* out_gn_steps) {
   if (h->last_n == 0) return MC_OK;
   MC_CUDA(cudaSetDevice(h->P.device));
   MC_CUDA(cudaMemcpyAsync(out_gn_steps, h->gn.p, sizeof(int64_t) * (size_t)h->last_n, cudaMemcpyDeviceToDevice, h->stream));
+  return MC_OK;
+}
+
+int mc_get_dissipation(mc_handle* h, double* out_wg) {
+  if (!h || !out_wg) return MC_EINVAL;
+  if (!(h->P.terms & MC_TERM_RR)) return MC_EINVAL;
+  if (h->last_n == 0) return MC_OK;
+  MC_CUDA(cudaSetDevice(h->P.device));
+  MC_CUDA(cudaMemcpyAsync(out_wg, h->diss.p, sizeof(double) * 4 * (size_t)h->last_n, cudaMemcpyDeviceToDevice, h->stream));
   return MC_OK;
 }
 
@@ -452,7 +472,7 @@ int mc_fp64_peak(int32_t device, double millis, double* out_tflops, double* out_
 int mc_destroy(mc_handle* h) {
   if (!h) return MC_EINVAL;
   cudaSetDevice(h->P.device);
-  h->status.release(); h->step.release(); h->gn.release();
+  h->status.release(); h->step.release(); h->gn.release(); h->diss.release();
   h->sched.release(); h->carry_d.release(); h->carry_i.release(); h->carry_g.release();
   h->h_in.release(); h->h_out.release(); h->h_inv.release(); h->h_fli.release();
   delete h;

@@ -21,7 +21,10 @@
 //   Omega1 = o1 u^3 L + 3 u^5 (m12 a2 + m11 a1) r - m12 u^3 sigma2     (= dH/dS1, S1 = s1 sigma1)
 //   Omega2 = o2 u^3 L + 3 u^5 (m21 a1 + m22 a2) r - m21 u^3 sigma1
 //   J = L + s1 sigma1 + s2 sigma2
-enum { MC_NCONST = 39 };
+// Radiation reaction (2.5PN, eq (6) of the paper; R21), force per unit mu with v = p at this order:
+//   F = u^3 [ (ra1 P + ra2 u + ra3 Q) (r.p) u^2 r - (rb1 P + rb2 u + rb3 Q) p ],  ra_i = (8/5) eta a_i, rb_i = (8/5) eta b_i,
+//   a = (3 + 3B, 23/3 + 2A - 3B, -5B), b = (2 + A, 2 - A, -3 - 3A) with the ADM gauge (A, B) = (5/3, 3)
+enum { MC_NCONST = 45 };
 enum McConstIndex {
   K_A1 = 0, K_B1, K_B2, K_H1, K_C3, K_D1, K_D2, K_D3, K_E1, K_E2, K_F1,  // orbital
   K_K1, K_K2, K_C12, K_Q1, K_Q2,                                         // spin couplings in H
@@ -29,7 +32,8 @@ enum McConstIndex {
   K_S1, K_S2,                                                            // spin magnitudes
   // fixed multiples of the above, so that no constant x constant product is left in the step loop
   K_2A1, K_3C3, K_2H1, K_3F1, K_2B2, K_2D2, K_4D3, K_2E2, K_2E1,         // 2 H_P, 2 H_Q, H_u polynomials
-  K_3C12, K_M5C12, K_3M12, K_3M21, K_3M11, K_3M22                         // spin-spin gradient / precession
+  K_3C12, K_M5C12, K_3M12, K_3M21, K_3M11, K_3M22,                        // spin-spin gradient / precession
+  K_RA1, K_RA2, K_RA3, K_RB1, K_RB2, K_RB3                                 // 2.5PN radiation reaction (MC_TERM_RR)
 };
 
 struct McConsts { double v[MC_NCONST]; };
@@ -80,4 +84,11 @@ MC_HD void mc_derive_consts(double beta, double chi1, double chi2, double kq1, d
   c[K_3M21 * stride] = 3.0 * c[K_M21 * stride];
   c[K_3M11 * stride] = 3.0 * c[K_M11 * stride];
   c[K_3M22 * stride] = 3.0 * c[K_M22 * stride];
+  const double rr = (terms & 32u) ? 1.6 * eta : 0.0, gA = 5.0 / 3.0, gB = 3.0;   // Schaefer's ADM gauge
+  c[K_RA1 * stride] = rr * (3.0 + 3.0 * gB);
+  c[K_RA2 * stride] = rr * (23.0 / 3.0 + 2.0 * gA - 3.0 * gB);
+  c[K_RA3 * stride] = rr * (-5.0 * gB);
+  c[K_RB1 * stride] = rr * (2.0 + gA);
+  c[K_RB2 * stride] = rr * (2.0 - gA);
+  c[K_RB3 * stride] = rr * (-3.0 - 3.0 * gA);
 }

@@ -42,7 +42,7 @@ MC_DEV int project_six(const C& c, T* z, const RefsT<T>& R, int iters, double to
     if (!warp_any(need)) break;
     if (need) {
       T g[12], H;
-      pn_eval<QM, false, true>(c, z, g, H);
+      pn_eval<QM, false, true, false>(c, z, g, H);
       T* r = z;
       T* p = z + 3;
       const T* a = g;

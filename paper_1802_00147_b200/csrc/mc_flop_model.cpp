@@ -37,13 +37,13 @@ mc_op_counts count(F f) {
   return delta(mc::op_counts(), before);
 }
 
-template <bool QM, int INTEG>
+template <bool QM, int INTEG, bool RR>
 void model(const HostConsts& c, int mode, int newton_iters, mc_flop_model_t* out) {
   using mc::Cnt;
-  Cnt z[12], f[12];
+  Cnt z[16], f[16];
   sample_state(z);
-  out->rhs = count([&] { mc::pn_rhs<QM>(c, z, f); });
-  out->base_step = count([&] { mc::base_step<INTEG, QM>(c, z, 1.0, f); });
+  out->rhs = count([&] { mc::pn_rhs<QM, RR>(c, z, f); });
+  out->base_step = count([&] { mc::base_step<INTEG, QM, RR>(c, z, 1.0, f); });
   mc::RefsT<Cnt> R;
   mc::references<QM>(c, z, R);
   out->references = count([&] { mc::references<QM>(c, z, R); });
@@ -84,19 +84,20 @@ void model(const HostConsts& c, int mode, int newton_iters, mc_flop_model_t* out
 
 extern "C" int mc_flop_model(uint32_t terms, int32_t correction_mode, int32_t integrator, int32_t newton_iters,
                              mc_flop_model_t* out) {
-  if (!out || (terms & ~31u) || correction_mode < 0 || correction_mode > 3) return MC_EINVAL;
+  if (!out || (terms & ~63u) || correction_mode < 0 || correction_mode > 3) return MC_EINVAL;
   if (integrator != MC_INTEG_RK4 && integrator != MC_INTEG_RK5) return MC_EINVAL;
   if (newton_iters < 1 || newton_iters > 16) return MC_EINVAL;
   HostConsts c;
   mc_derive_consts(0.8, 0.9, 0.7, 2.0, 3.0, terms, c.v);
   const bool qm = (terms & MC_TERM_QM) != 0;
   memset(out, 0, sizeof(*out));
-  if (qm) {
-    if (integrator == MC_INTEG_RK5) model<true, 1>(c, correction_mode, newton_iters, out);
-    else model<true, 0>(c, correction_mode, newton_iters, out);
+  const bool rr = (terms & MC_TERM_RR) != 0, rk5 = integrator == MC_INTEG_RK5;
+  if (rr) {
+    if (qm) { if (rk5) model<true, 1, true>(c, correction_mode, newton_iters, out); else model<true, 0, true>(c, correction_mode, newton_iters, out); }
+    else { if (rk5) model<false, 1, true>(c, correction_mode, newton_iters, out); else model<false, 0, true>(c, correction_mode, newton_iters, out); }
   } else {
-    if (integrator == MC_INTEG_RK5) model<false, 1>(c, correction_mode, newton_iters, out);
-    else model<false, 0>(c, correction_mode, newton_iters, out);
+    if (qm) { if (rk5) model<true, 1, false>(c, correction_mode, newton_iters, out); else model<true, 0, false>(c, correction_mode, newton_iters, out); }
+    else { if (rk5) model<false, 1, false>(c, correction_mode, newton_iters, out); else model<false, 0, false>(c, correction_mode, newton_iters, out); }
   }
   return MC_OK;
 }

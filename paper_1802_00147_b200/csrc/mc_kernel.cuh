@@ -42,7 +42,8 @@ struct IntegrateArgs {
   // scheduling
   unsigned long long* queue;  // [0] = next item
   int32_t* done;              // [n_units] chunks completed per unit
-  double* carry_d;            // [17][n_traj_padded]: y[12], E0, J0[3], acc
+  double* carry_d;            // [17][n_traj_padded]: y[12], E0, J0[3] (MC_TERM_RR: E0 + W, J0 + G), acc
+  double* out_diss;           // [4][n]: E0 + W, J0 + G of the orbit at the end (MC_TERM_RR), handle-owned
   int32_t* carry_i;           // [2][n_traj_padded]: status | flag << 8 | frozen << 31, until_renorm
   unsigned long long* carry_g;  // [2][n_traj_padded]: Gauss-Newton steps, completed steps (64-bit: they accumulate over resumed calls)
   int64_t n_units;            // ceil(trajectories / 32)
@@ -98,9 +99,14 @@ template <int PARAMS> struct ConstsOf { typedef UniformConsts type; };
 template <> struct ConstsOf<PARAMS_PER_ORBIT> { typedef SharedConsts type; };
 template <> struct ConstsOf<PARAMS_KAPPA> { typedef KappaConsts type; };
 
-template <int PARAMS, bool QM, int MODE, int INTEG, int MINB>
+// RR: 2.5PN radiation reaction (MC_TERM_RR): the correction targets E0 + W, J0 + G, W and G being the work and torque
+// integrals of the force (R21).  W and G enter nowhere else, so the trajectory carries the
+// MOVING REFERENCES themselves as components 12-15 through the RK step (initial values E0, J0, rates dW/dt, dG/dt)
+// and the separate reference registers R are not used.
+template <int PARAMS, bool QM, int MODE, int INTEG, bool RR, int MINB>
 __global__ void MC_KERNEL_BOUNDS(MINB)
 integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ IntegrateArgs A) {
+  constexpr int NS = RR ? 16 : 12;
   extern __shared__ double smem[];   // PARAMS_PER_ORBIT: [MC_NCONST][kBlock]
   const bool shadow = A.shadow_eps != 0.0;
   const int lane = threadIdx.x & 31;
@@ -125,7 +131,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
     using CP = typename ConstsOf<PARAMS>::type;
     const CP c = make_consts<PARAMS, CP>(uc, A, orbit, smem);
 
-    double y[12];
+    double y[NS];
     Refs R;
     int status = ST_OK, flag = 0;
     bool frozen = false;
@@ -149,6 +155,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
       }
       if (role_shadow) y[0] += A.shadow_eps;
       references<QM>(c, y, R);
+      if constexpr (RR) { y[12] = R.E0; y[13] = R.J0[0]; y[14] = R.J0[1]; y[15] = R.J0[2]; }
     } else {
       // wait until this unit's previous chunk is published, then reload the carried state.  The holder of
       // that chunk got it earlier from the same queue, so it is running -- PROVIDED the whole grid is resident at
@@ -173,6 +180,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
 #pragma unroll
       for (int i = 0; i < 3; ++i) R.J0[i] = __ldcg(A.carry_d + (int64_t)(13 + i) * tp + t);
       acc = __ldcg(A.carry_d + 16 * tp + t);
+      if constexpr (RR) { y[12] = R.E0; y[13] = R.J0[0]; y[14] = R.J0[1]; y[15] = R.J0[2]; }
       const int packed = __ldcg(A.carry_i + t);
       status = packed & 0xff;
       flag = (packed >> 8) & ST_NEWTON_FLAG;   // bit 16 -> 256
@@ -196,10 +204,17 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
         }
         break;
       }
-      double z[12];
-      base_step<INTEG, QM>(c, y, A.h, z);
+      double z[NS];
+      base_step<INTEG, QM, RR>(c, y, A.h, z);
       int gn;
-      const bool ok = correct<MODE, QM>(c, z, R, A.newton_iters, A.newton_tol, gn);
+      bool ok;
+      if constexpr (RR) {   // the manifold has moved by the work and torque of the step (integral invariant relation)
+        Refs Rm;
+        Rm.E0 = z[12]; Rm.J0[0] = z[13]; Rm.J0[1] = z[14]; Rm.J0[2] = z[15];
+        ok = correct<MODE, QM>(c, z, Rm, A.newton_iters, A.newton_tol, gn);
+      } else {
+        ok = correct<MODE, QM>(c, z, R, A.newton_iters, A.newton_tol, gn);
+      }
       if (MODE == 2 && !ok && !role_shadow && !frozen) flag = ST_NEWTON_FLAG;
       // status of the completed step (R13): non-finite anywhere in the pair, else |r| of the main
       int code = ST_OK;
@@ -215,7 +230,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
       if (!frozen) {
         if (code == ST_OK) {
 #pragma unroll
-          for (int i = 0; i < 12; ++i) y[i] = z[i];
+          for (int i = 0; i < NS; ++i) y[i] = z[i];
           ++steps;
           gn_chunk += (unsigned)gn;
         } else {
@@ -253,6 +268,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
             for (int i = 0; i < 12; ++i) y[i] = fma(s, y[i] - ym[i], ym[i]);
             if (MODE >= 1) { normalise3(y + 6); normalise3(y + 9); }
             references<QM>(c, y, R);   // the shadow obeys its own, re-referenced integrals (R11)
+            if constexpr (RR) { y[12] = R.E0; y[13] = R.J0[0]; y[14] = R.J0[1]; y[15] = R.J0[2]; }   // W, G restart with them
           }
         }
         bad |= __shfl_xor_sync(0xffffffffu, bad, 1);
@@ -272,6 +288,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
       // park the state in the carry buffer (and publish the chunk unless it is the last)
 #pragma unroll
       for (int i = 0; i < 12; ++i) __stcg(A.carry_d + (int64_t)i * tp + t, y[i]);
+      if constexpr (RR) { R.E0 = y[12]; R.J0[0] = y[13]; R.J0[1] = y[14]; R.J0[2] = y[15]; }
       __stcg(A.carry_d + 12 * tp + t, R.E0);
 #pragma unroll
       for (int i = 0; i < 3; ++i) __stcg(A.carry_d + (int64_t)(13 + i) * tp + t, R.J0[i]);
@@ -310,6 +327,10 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
         six_integrals<QM>(c, y, inv1);
 #pragma unroll
         for (int i = 0; i < 6; ++i) A.out_inv[(int64_t)(6 + i) * A.n + orbit] = inv1[i];
+      }
+      if constexpr (RR) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) A.out_diss[(int64_t)i * A.n + orbit] = y[12 + i];
       }
       A.out_status[orbit] = status | flag;
       A.out_step[orbit] = steps_total;

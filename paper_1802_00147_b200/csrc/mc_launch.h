@@ -11,8 +11,8 @@ struct KernelInfo { int regs, local_bytes, blocks_per_sm, block, grid; size_t sm
 // query: fills KernelInfo (occupancy, registers) without launching.  launch: starts min(blocks needed,
 // resident capacity) persistent blocks.
 typedef cudaError_t (*LaunchFn)(const McConsts&, const IntegrateArgs&, int num_sms, bool do_launch, cudaStream_t, KernelInfo*);
-LaunchFn launcher_mode0(int params, bool qm, int integrator);
-LaunchFn launcher_mode1(int params, bool qm, int integrator);
-LaunchFn launcher_mode2(int params, bool qm, int integrator);
-LaunchFn launcher_mode3(int params, bool qm, int integrator);
+LaunchFn launcher_mode0(int params, bool qm, int integrator, bool rr);
+LaunchFn launcher_mode1(int params, bool qm, int integrator, bool rr);
+LaunchFn launcher_mode2(int params, bool qm, int integrator, bool rr);
+LaunchFn launcher_mode3(int params, bool qm, int integrator, bool rr);
 }  // namespace mc

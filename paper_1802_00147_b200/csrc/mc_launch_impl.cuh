@@ -19,10 +19,10 @@ namespace mc {
 #define MC_MINB_PER_ORBIT 2
 #endif
 
-template <int PARAMS, bool QM, int MODE, int INTEG>
+template <int PARAMS, bool QM, int MODE, int INTEG, bool RR>
 static cudaError_t launch(const McConsts& uc, const IntegrateArgs& A, int num_sms, bool do_launch, cudaStream_t stream,
                           KernelInfo* info) {
-  auto kern = integrate_kernel<PARAMS, QM, MODE, INTEG, ((PARAMS == PARAMS_PER_ORBIT || INTEG == 1) ? MC_MINB_PER_ORBIT : MC_MINB_UNIFORM)>;
+  auto kern = integrate_kernel<PARAMS, QM, MODE, INTEG, RR, ((PARAMS == PARAMS_PER_ORBIT || INTEG == 1 || RR) ? MC_MINB_PER_ORBIT : MC_MINB_UNIFORM)>;
   const size_t smem = PARAMS == PARAMS_PER_ORBIT ? sizeof(double) * MC_NCONST * kBlock : 0;
   cudaFuncAttributes fa;
   cudaError_t e = cudaFuncGetAttributes(&fa, kern);
@@ -47,17 +47,23 @@ static cudaError_t launch(const McConsts& uc, const IntegrateArgs& A, int num_sm
 }
 
 // params: 0 uniform, 1 per orbit, 2 per-orbit kappa only (meaningful with the QM term; without it kappa is unused
-// and the uniform kernel runs)
-template <int MODE, int INTEG>
-static LaunchFn pick2(int params, bool qm) {
-  if (params == PARAMS_PER_ORBIT) return qm ? launch<PARAMS_PER_ORBIT, true, MODE, INTEG> : launch<PARAMS_PER_ORBIT, false, MODE, INTEG>;
-  if (params == PARAMS_KAPPA && qm) return launch<PARAMS_KAPPA, true, MODE, INTEG>;
-  return qm ? launch<PARAMS_UNIFORM, true, MODE, INTEG> : launch<PARAMS_UNIFORM, false, MODE, INTEG>;
+// and the uniform kernel runs); rr: 2.5PN radiation reaction (16-component trajectories)
+template <int MODE, int INTEG, bool RR>
+static LaunchFn pick3(int params, bool qm) {
+  if (params == PARAMS_PER_ORBIT) {
+    // 37 per-orbit constants + six RK5 stages + the 16-component trajectory do not fit 255 registers: that one
+    // combination is not built (mc_integrate returns MC_EINVAL; include/mc.h, MC_TERM_RR)
+    if constexpr (INTEG == 1 && RR) return nullptr;
+    else return qm ? launch<PARAMS_PER_ORBIT, true, MODE, INTEG, RR> : launch<PARAMS_PER_ORBIT, false, MODE, INTEG, RR>;
+  }
+  if (params == PARAMS_KAPPA && qm) return launch<PARAMS_KAPPA, true, MODE, INTEG, RR>;
+  return qm ? launch<PARAMS_UNIFORM, true, MODE, INTEG, RR> : launch<PARAMS_UNIFORM, false, MODE, INTEG, RR>;
 }
 
 template <int MODE>
-static LaunchFn pick(int params, bool qm, int integrator) {
-  return integrator == 1 ? pick2<MODE, 1>(params, qm) : pick2<MODE, 0>(params, qm);
+static LaunchFn pick(int params, bool qm, int integrator, bool rr) {
+  if (rr) return integrator == 1 ? pick3<MODE, 1, true>(params, qm) : pick3<MODE, 0, true>(params, qm);
+  return integrator == 1 ? pick3<MODE, 1, false>(params, qm) : pick3<MODE, 0, false>(params, qm);
 }
 
 }  // namespace mc

@@ -98,8 +98,12 @@ MC_DEV void cross3(const T* a, const T* b, T* c) {
 // ---- the fused model routine ----------------------------------------------------------------------
 // Input  z = (r[0:3], p[3:6], sigma1[6:9], sigma2[9:12]).
 // Output g[0:3] = dH/dr, g[3:6] = dH/dp; if OMEGA: g[6:9] = Omega1, g[9:12] = Omega2; if WANT_H: H.
+// With RR (2.5PN radiation reaction, MC_TERM_RR; only the equations of motion use it): g[0:3] = dH/dr - F, so that
+// dp/dt = -g as in the conservative case, and g[12] = (dH/dp).F, g[13:16] = r x F, the rates of the work and torque
+// integrals W, G.  F = fr r + fp p has no other components, so it costs two coefficients:
+// r x F = fp L, v.F = fr (v.r) + fp (v.p) with v.r = A (r.p) + B r^2, v.p = A P + B (r.p) + H_SO.
 // eqs (1)-(9) of the paper with the readings of DESIGN.md section 3.
-template <bool QM, bool OMEGA, bool WANT_H, class C, class T>
+template <bool QM, bool OMEGA, bool WANT_H, bool RR, class C, class T>
 MC_DEV void pn_eval(const C& c, const T* z, T* g, T& H) {
   const T* r = z;
   const T* p = z + 3;
@@ -160,10 +164,21 @@ MC_DEV void pn_eval(const C& c, const T* z, T* g, T& H) {
     w2 = fma(6.0, q2a, w2);
     if (WANT_H) Hss += fma(3.0, q1aa, -(q1u3 * d11)) + fma(3.0, q2aa, -(q2u3 * d22));
   }
-  const T Cr = u2 * fma(3.0, X, -Cu);                 // coefficient of r in dH/dr
+  T Cr = u2 * fma(3.0, X, -Cu);                       // coefficient of r in dH/dr
+  T Bp = B;                                           // coefficient of p in dH/dr
+  if constexpr (RR) {
+    const T ca = fma(c[K_RA3], Q, fma(c[K_RA2], u, c[K_RA1] * P));
+    const T cb = fma(c[K_RB3], Q, fma(c[K_RB2], u, c[K_RB1] * P));
+    const T fr = ca * w * u3, fp = -(cb * u3);         // F = fr r + fp p
+    Cr -= fr;
+    Bp -= fp;
+    g[12] = fma(fr, fma(A, rp, B * r2), fp * fma(A, P, fma(B, rp, LS)));
+#pragma unroll
+    for (int i = 0; i < 3; ++i) g[13 + i] = fp * L[i];
+  }
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
-    g[i] = fma(w2, s2[i], fma(w1, s1[i], fma(Cr, r[i], fma(B, p[i], PxS[i]))));
+    g[i] = fma(w2, s2[i], fma(w1, s1[i], fma(Cr, r[i], fma(Bp, p[i], PxS[i]))));
     g[3 + i] = fma(A, p[i], fma(B, r[i], SxR[i]));
   }
   if (OMEGA) {
@@ -186,15 +201,20 @@ MC_DEV void pn_eval(const C& c, const T* z, T* g, T& H) {
   }
 }
 
-// dz/dt, eqs (6)-(7): dr/dt = dH/dp, dp/dt = -dH/dr, dsigma_i/dt = Omega_i x sigma_i.
-template <bool QM, class C, class T>
+// dz/dt, eqs (6)-(7): dr/dt = dH/dp, dp/dt = -dH/dr (+ a_2.5PN), dsigma_i/dt = Omega_i x sigma_i.
+// RR: 16 components, f[12] = dW/dt, f[13:16] = dG/dt.
+template <bool QM, bool RR, class C, class T>
 MC_DEV void pn_rhs(const C& c, const T* z, T* f) {
-  T g[12], H;
-  pn_eval<QM, true, false>(c, z, g, H);
+  T g[RR ? 16 : 12], H;
+  pn_eval<QM, true, false, RR>(c, z, g, H);
 #pragma unroll
   for (int i = 0; i < 3; ++i) { f[i] = g[3 + i]; f[3 + i] = -g[i]; }
   cross3(g + 6, z + 6, f + 6);
   cross3(g + 9, z + 9, f + 9);
+  if constexpr (RR) {
+#pragma unroll
+    for (int i = 12; i < 16; ++i) f[i] = g[i];
+  }
 }
 
 // J = r x p + s1 sigma1 + s2 sigma2
@@ -208,42 +228,56 @@ MC_DEV void total_J(const C& c, const T* z, T* J) {
 template <bool QM, class C, class T>
 MC_DEV T hamiltonian(const C& c, const T* z) {
   T g[12], H;
-  pn_eval<QM, false, true>(c, z, g, H);
+  pn_eval<QM, false, true, false>(c, z, g, H);
   return H;
 }
 
 // Classical RK4 (R9), low-storage bookkeeping: y (kept), acc, stage input yt.
-template <bool QM, class C, class T>
+// RR: components 12-15 (W, G) never enter the right-hand side, so they need no stage inputs: only their weighted
+// sum of stage derivatives is accumulated.
+template <bool QM, bool RR, class C, class T>
 MC_DEV void rk4_step(const C& c, const T* y, double h, T* out) {
+  constexpr int NS = RR ? 16 : 12;
   const double h2 = 0.5 * h, h3 = h * (1.0 / 3.0), h6 = h * (1.0 / 6.0);
-  T k[12], yt[12];
-  pn_rhs<QM>(c, y, k);
+  T k[NS], yt[12];
+  pn_rhs<QM, RR>(c, y, k);
 #pragma unroll
-  for (int i = 0; i < 12; ++i) { out[i] = fma(h6, k[i], y[i]); yt[i] = fma(h2, k[i], y[i]); }
-  pn_rhs<QM>(c, yt, k);
+  for (int i = 0; i < NS; ++i) out[i] = fma(h6, k[i], y[i]);
 #pragma unroll
-  for (int i = 0; i < 12; ++i) { out[i] = fma(h3, k[i], out[i]); yt[i] = fma(h2, k[i], y[i]); }
-  pn_rhs<QM>(c, yt, k);
+  for (int i = 0; i < 12; ++i) yt[i] = fma(h2, k[i], y[i]);
+  pn_rhs<QM, RR>(c, yt, k);
 #pragma unroll
-  for (int i = 0; i < 12; ++i) { out[i] = fma(h3, k[i], out[i]); yt[i] = fma(h, k[i], y[i]); }
-  pn_rhs<QM>(c, yt, k);
+  for (int i = 0; i < NS; ++i) out[i] = fma(h3, k[i], out[i]);
 #pragma unroll
-  for (int i = 0; i < 12; ++i) out[i] = fma(h6, k[i], out[i]);
+  for (int i = 0; i < 12; ++i) yt[i] = fma(h2, k[i], y[i]);
+  pn_rhs<QM, RR>(c, yt, k);
+#pragma unroll
+  for (int i = 0; i < NS; ++i) out[i] = fma(h3, k[i], out[i]);
+#pragma unroll
+  for (int i = 0; i < 12; ++i) yt[i] = fma(h, k[i], y[i]);
+  pn_rhs<QM, RR>(c, yt, k);
+#pragma unroll
+  for (int i = 0; i < NS; ++i) out[i] = fma(h6, k[i], out[i]);
 }
 
 // Butcher's six-stage fifth-order method (the paper's "RK5", R9):
 //   c = 0, 1/4, 1/4, 1/2, 3/4, 1;  b = 7/90, 0, 32/90, 12/90, 32/90, 7/90
 //   a2 = (1/4); a3 = (1/8, 1/8); a4 = (0, -1/2, 1); a5 = (3/16, 0, 0, 9/16); a6 = (-3/7, 2/7, 12/7, -12/7, 8/7)
 // Bookkeeping: the linear combinations needed later (stage-4 input, stage-6 input, final sum) are accumulated as
-// the stages arrive, so at most five 12-vectors are live besides the derivative being computed.
-template <bool QM, class C, class T>
+// the stages arrive, so at most five 12-vectors are live besides the derivative being computed.  RR: components
+// 12-15 only accumulate the final sum (see rk4_step).
+template <bool QM, bool RR, class C, class T>
 MC_DEV void rk5_step(const C& c, const T* y, double h, T* out) {
-  T k[12], k1[12], yt[12], A4[12], S6[12];
-  pn_rhs<QM>(c, y, k1);
+  constexpr int NS = RR ? 16 : 12;
+  T k[NS], k1[12], yt[12], A4[12], S6[12];
+  const double h790 = h * (7.0 / 90.0), h3290 = h * (32.0 / 90.0), h1290 = h * (12.0 / 90.0);
+  pn_rhs<QM, RR>(c, y, k);
   const double h4 = 0.25 * h, h8 = 0.125 * h;
 #pragma unroll
-  for (int i = 0; i < 12; ++i) yt[i] = fma(h4, k1[i], y[i]);
-  pn_rhs<QM>(c, yt, k);                                                    // k2
+  for (int i = 0; i < 12; ++i) { k1[i] = k[i]; yt[i] = fma(h4, k[i], y[i]); }
+#pragma unroll
+  for (int i = 12; i < NS; ++i) out[i] = fma(h790, k[i], y[i]);
+  pn_rhs<QM, RR>(c, yt, k);                                                    // k2 (b2 = 0)
   const double hm2 = -0.5 * h, h37 = h * (-3.0 / 7.0), h27 = h * (2.0 / 7.0);
 #pragma unroll
   for (int i = 0; i < 12; ++i) {
@@ -251,39 +285,41 @@ MC_DEV void rk5_step(const C& c, const T* y, double h, T* out) {
     A4[i] = fma(hm2, k[i], y[i]);
     S6[i] = fma(h27, k[i], fma(h37, k1[i], y[i]));
   }
-  pn_rhs<QM>(c, yt, k);                                                    // k3
-  const double h127 = h * (12.0 / 7.0), h790 = h * (7.0 / 90.0), h3290 = h * (32.0 / 90.0);
+  pn_rhs<QM, RR>(c, yt, k);                                                    // k3
+  const double h127 = h * (12.0 / 7.0);
 #pragma unroll
   for (int i = 0; i < 12; ++i) {
     yt[i] = fma(h, k[i], A4[i]);
     S6[i] = fma(h127, k[i], S6[i]);
     out[i] = fma(h3290, k[i], fma(h790, k1[i], y[i]));
   }
-  pn_rhs<QM>(c, yt, k);                                                    // k4
-  const double h316 = h * (3.0 / 16.0), h916 = h * (9.0 / 16.0), h1290 = h * (12.0 / 90.0);
+#pragma unroll
+  for (int i = 12; i < NS; ++i) out[i] = fma(h3290, k[i], out[i]);
+  pn_rhs<QM, RR>(c, yt, k);                                                    // k4
+  const double h316 = h * (3.0 / 16.0), h916 = h * (9.0 / 16.0);
 #pragma unroll
   for (int i = 0; i < 12; ++i) {
     yt[i] = fma(h916, k[i], fma(h316, k1[i], y[i]));
     S6[i] = fma(-h127, k[i], S6[i]);
-    out[i] = fma(h1290, k[i], out[i]);
   }
-  pn_rhs<QM>(c, yt, k);                                                    // k5
+#pragma unroll
+  for (int i = 0; i < NS; ++i) out[i] = fma(h1290, k[i], out[i]);
+  pn_rhs<QM, RR>(c, yt, k);                                                    // k5
   const double h87 = h * (8.0 / 7.0);
 #pragma unroll
-  for (int i = 0; i < 12; ++i) {
-    yt[i] = fma(h87, k[i], S6[i]);
-    out[i] = fma(h3290, k[i], out[i]);
-  }
-  pn_rhs<QM>(c, yt, k);                                                    // k6
+  for (int i = 0; i < 12; ++i) yt[i] = fma(h87, k[i], S6[i]);
 #pragma unroll
-  for (int i = 0; i < 12; ++i) out[i] = fma(h790, k[i], out[i]);
+  for (int i = 0; i < NS; ++i) out[i] = fma(h3290, k[i], out[i]);
+  pn_rhs<QM, RR>(c, yt, k);                                                    // k6
+#pragma unroll
+  for (int i = 0; i < NS; ++i) out[i] = fma(h790, k[i], out[i]);
 }
 
 // INTEG: 0 classical RK4, 1 Butcher RK5
-template <int INTEG, bool QM, class C, class T>
+template <int INTEG, bool QM, bool RR, class C, class T>
 MC_DEV void base_step(const C& c, const T* y, double h, T* out) {
-  if (INTEG == 1) rk5_step<QM>(c, y, h, out);
-  else rk4_step<QM>(c, y, h, out);
+  if (INTEG == 1) rk5_step<QM, RR>(c, y, h, out);
+  else rk4_step<QM, RR>(c, y, h, out);
 }
 
 // eq (10): sigma <- sigma / |sigma|

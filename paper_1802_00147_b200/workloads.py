@@ -12,7 +12,7 @@ from dataclasses import dataclass, field
 import numpy as np
 
 SEED_BASE = 1802001470
-TERM_1PN, TERM_2PN, TERM_SO, TERM_S1S2, TERM_QM = 1, 2, 4, 8, 16
+TERM_1PN, TERM_2PN, TERM_SO, TERM_S1S2, TERM_QM, TERM_RR = 1, 2, 4, 8, 16, 32
 TERMS_DEFAULT = TERM_1PN | TERM_2PN | TERM_SO | TERM_S1S2
 
 

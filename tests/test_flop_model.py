@@ -42,6 +42,19 @@ def test_terms_and_modes_add_what_they_should():
     assert 20 <= per_iter <= 40                                                        # one Horner pair + division per iteration
 
 
+def test_radiation_reaction_adds_the_force_and_four_accumulations():
+    """MC_TERM_RR: the force costs two coefficients (F = fr r + fp p) plus the rates dW/dt, dG/dt, and the RK step
+    accumulates four more components (no stage inputs for them: they never enter the right-hand side)."""
+    a, b = binding.flop_model(15, 3, RK4), binding.flop_model(15 | 32, 3, RK4)
+    extra = b["rhs"]["flop"] - a["rhs"]["flop"]
+    assert 20 <= extra <= 40 and b["rhs"]["special"] == 1
+    assert b["base_step"]["flop"] == 4 * b["rhs"]["flop"] + 2 * (84 + 4 * 4)
+    b5 = binding.flop_model(15 | 32, 3, RK5)
+    assert b5["base_step"]["flop"] == 6 * b["rhs"]["flop"] + 2 * (204 + 5 * 4)          # b2 = 0: five accumulations
+    assert b["gn_step"] == a["gn_step"]                                                # the projection uses grad H only
+    assert b["correct_fixed"]["flop"] == a["correct_fixed"]["flop"]                    # the references are carried, not added
+
+
 def test_kernel_formulation_needs_less_work_than_the_oracles():
     """the oracle's unfactored formulation costs about twice as much; using the kernel's own count for
     `roofline.achieved` is the conservative choice."""

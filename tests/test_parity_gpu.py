@@ -734,3 +734,121 @@ def test_config4_maximum_size_properties(mc):
     assert np.abs(I1[0] / inv[0, : n // 2] - 1).max() <= DRIFT_TOL
     assert (np.linalg.norm(I1[1:4] - inv[1:4, : n // 2], axis=0) / np.linalg.norm(inv[1:4, : n // 2], axis=0)).max() <= DRIFT_TOL
     assert np.abs(inv[6:12, : n // 2] - I1).max() < 1e-13                    # the kernel's own final invariants agree
+
+
+RR = workloads.TERM_RR
+
+
+@pytest.mark.parametrize("terms", [RR, 15 | RR, 31 | RR])
+def test_radiation_reaction_model_routines_match_oracle(mc, terms):
+    """SURVEY 8(f) row 4 (MC_TERM_RR; eq 6; R21): dz/dt with the 2.5PN force and the rates
+    of the work and torque integrals (16 rows), one RK4 / RK5 step of all 16 components."""
+    z = random_states(300, seed=31)
+    par = PARAM_SETS[1]
+    for integ, ointeg in ((mc.MC_INTEG_RK4, oracle.RK4), (mc.MC_INTEG_RK5, oracle.RK5)):
+        with mc.Integrator(terms=terms, integrator=integ, **par) as I:
+            got = I.eval("rhs", z).cpu().numpy()
+            step = I.eval("rk4_step", z, h=1.0).cpu().numpy()
+        want = oracle.evaluate("rhs16", z, terms=terms, **par)
+        assert got.shape == (16, 300)
+        assert rel_state_err_blocks(got[0:12], want[0:12]) < 2e-13
+        assert np.abs(got[12] / want[12] - 1).max() < 1e-12                           # dW/dt
+        assert (np.linalg.norm(got[13:16] - want[13:16], axis=0) / np.linalg.norm(want[13:16], axis=0)).max() < 1e-12
+        plain = oracle.rhs(z, terms=terms & ~RR, **par)
+        assert rel_state_err_blocks(got[3:6], plain[3:6]) > 1e-9                      # the force really is in dp/dt
+        o = oracle.integrate(z, 1.0, 1, 0, terms=terms, integrator=ointeg, r_merge=0.0, r_escape=1e9, **par)
+        assert rel_state_err_blocks(step[0:12], o.states) < 2e-13
+        assert np.abs(step[12] / o.diss[0] - 1).max() < 1e-11 and np.abs(step[13:16] - o.diss[1:4]).max() < 1e-13 * np.abs(o.diss[1:4]).max()
+
+
+@pytest.mark.parametrize("mode", [0, 2, 3])
+def test_radiation_reaction_runs_match_oracle(mc, mode):
+    """Dissipative runs: config-0 orbits and the paper's orbit 3 with the 2.5PN term, shadow on.  State
+    parity, status, FLI, and the moving references E0 + W, J0 + G (mc_get_dissipation) against the oracle's W, G;
+    with the correction the integral invariant relation holds to round-off on the GPU's output (oracle-evaluated)."""
+    w = workloads.config0(149)
+    z = np.concatenate([w.states, workloads.paper_orbit(3).states], axis=1)
+    par = dict(beta=1.0, chi1=1.0, chi2=0.85)
+    terms = 15 | RR
+    n = z.shape[1]
+    with mc.Integrator(terms=terms, **par) as I:
+        g = I.integrate(z, 1.0, 1000, mode, shadow_eps=1e-8)
+        ref = I.dissipation(n).cpu().numpy()
+        info = I.launch_info()
+    with mc.Integrator(terms=terms, chunk_steps=170, **par) as I:
+        gc = I.integrate(z, 1.0, 1000, mode, shadow_eps=1e-8)
+        refc = I.dissipation(n).cpu().numpy()
+    o = oracle.integrate(z, 1.0, 1000, mode, shadow_eps=1e-8, terms=terms, **par)
+    assert info["local_bytes"] == 0 and info["variant"] & 8
+    gz, ginv = g.states.cpu().numpy(), g.invariants.cpu().numpy()
+    assert np.array_equal(g.status.cpu().numpy() & 255, o.status & 255) and (o.status & 255 == 0).all()
+    clean = o.status == 0                                                              # mode 2: no skipped step (R7)
+    assert clean.sum() >= (30 if mode == 2 else n)
+    assert rel_state_err(gz[:, clean], o.states[:, clean]) <= (2e-9 if mode == 2 else STATE_RTOL)
+    assert np.abs(g.fli.cpu().numpy()[clean] - o.fli[clean]).max() < (1e-2 if mode == 2 else 1e-3)
+    W = ref[0] - ginv[0]
+    G = ref[1:4] - ginv[1:4]
+    assert (W < 0).all()                                                               # energy is radiated
+    assert np.abs(W[clean] / o.diss[0][clean] - 1).max() < 1e-6                        # E0 + W carries 1e-16 E0 of rounding, W ~ 1e-7 E0
+    assert (np.linalg.norm(G - o.diss[1:4], axis=0) / np.linalg.norm(o.diss[1:4], axis=0))[clean].max() < 1e-6
+    I1 = oracle.integrals(gz, terms=terms, **par)
+    resE = np.abs(I1[0] - ref[0]) / np.abs(ginv[0])
+    resJ = np.linalg.norm(I1[1:4] - ref[1:4], axis=0) / np.linalg.norm(ginv[1:4], axis=0)
+    if mode == 3:
+        assert resE.max() <= DRIFT_TOL and resJ.max() <= DRIFT_TOL                     # integral invariant relation, PAPER.md:221
+    elif mode == 2:
+        assert resE[clean].max() <= DRIFT_TOL
+    else:
+        assert 1e-14 < resE.max() < 1e-6                                               # uncorrected: truncation error only
+    assert np.array_equal(gz, gc.states.cpu().numpy()) and np.array_equal(ref, refc)   # chunking never changes a bit
+    assert np.array_equal(g.fli.cpu().numpy(), gc.fli.cpu().numpy())
+
+
+def test_radiation_reaction_variants_and_resume(mc):
+    """The other instantiations of the dissipative kernel: per-orbit parameters, per-orbit kappa + QM, RK5; checkpoint /
+    resume carries the moving references; the one combination that is not built is refused."""
+    w = workloads.config3(n_r=6, n_theta=11, qm=True)
+    kw = {k: v for k, v in w.params().items() if k != "terms"}
+    terms = w.terms | RR
+    o = oracle.integrate(w.states, 1.0, 600, 3, shadow_eps=1e-8, **dict(w.params(), terms=terms))
+    ok = o.status == 0
+    assert ok.sum() > 30
+    for force in (None, 1):
+        with mc.Integrator(terms=terms, per_orbit=force, **kw) as I:
+            g = I.integrate(w.states, 1.0, 600, 3, shadow_eps=1e-8)
+            ref = I.dissipation(w.n_orbits).cpu().numpy()
+            assert I.launch_info()["local_bytes"] == 0
+        assert np.array_equal(g.status.cpu().numpy(), o.status)
+        assert rel_state_err(g.states.cpu().numpy()[:, ok], o.states[:, ok]) <= STATE_RTOL
+        W = ref[0] - g.invariants.cpu().numpy()[0]
+        assert np.abs(W[ok] / o.diss[0][ok] - 1).max() < 1e-6
+    o5 = oracle.integrate(w.states, 1.0, 600, 3, shadow_eps=1e-8, integrator=oracle.RK5, **dict(w.params(), terms=terms))
+    with mc.Integrator(terms=terms, integrator=mc.MC_INTEG_RK5, **kw) as I:
+        one = I.integrate(w.states, 1.0, 600, 3, shadow_eps=1e-8)
+        one_ref = I.dissipation(w.n_orbits).cpu().numpy()
+        a = I.integrate_ex(w.states, 1.0, 250, 3, shadow_eps=1e-8)
+        b = I.integrate_ex(None, 1.0, 350, 3, shadow_eps=1e-8, carry=a.carry, resume=True, n_orbits=w.n_orbits, invariants=a.invariants)
+        b_ref = I.dissipation(w.n_orbits).cpu().numpy()
+    ok5 = o5.status == 0
+    assert rel_state_err(one.states.cpu().numpy()[:, ok5], o5.states[:, ok5]) <= STATE_RTOL
+    assert np.array_equal(one.states.cpu().numpy(), b.states.cpu().numpy()) and np.array_equal(one_ref, b_ref)
+    assert np.array_equal(one.fli.cpu().numpy(), b.fli.cpu().numpy(), equal_nan=True)
+    with mc.Integrator(terms=terms, integrator=mc.MC_INTEG_RK5, per_orbit=1, **kw) as I:   # not built: register budget (mc.h)
+        with pytest.raises(mc.MCError) as e:
+            I.integrate(w.states, 1.0, 10, 3, shadow_eps=1e-8)
+        assert e.value.code == mc.MC_EINVAL
+    with mc.Integrator(terms=w.terms, **kw) as I:                                       # without the bit: no dissipation output
+        I.integrate(w.states, 1.0, 10, 3, shadow_eps=1e-8)
+        with pytest.raises(mc.MCError):
+            I.dissipation(w.n_orbits)
+
+
+def test_mc_eval_rejects_null_references(mc):
+    """mc_eval(what = 4) reads refs for every mode; a NULL must be MC_EINVAL, not a device fault."""
+    z = random_states(40, seed=2)
+    with mc.Integrator() as I:
+        for mode in (0, 1, 2, 3):
+            with pytest.raises(mc.MCError) as e:
+                I.eval("correct", z, mode=mode, refs=None)
+            assert e.value.code == mc.MC_EINVAL
+        assert I.eval("H", z).shape == (1, 40)                                           # the handle is still usable

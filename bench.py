@@ -128,6 +128,33 @@ def algorithmic_flop(w, mode, integrator, steps_done, gn_steps):
             "per_trajectory_step_without_gn": per_traj_step}
 
 
+def executed_from_sass(w, rk5, warp_work, per_launch_s, num_sms, sm_mhz, value):
+    """What the device executed in one launch, from the SASS instruction mix of the step loop (sass_mix.py, read from
+    the library's own object file) times the warp-level work counters of the launch (mc_get_warp_work), and the time
+    the FP64 pipe needs for it under the measured operand-bandwidth rule (3 cycles for an FMA with three distinct
+    register operands, 2 otherwise; mc_fp64_probe).  None for kernels the SASS reader does not handle."""
+    from paper_1802_00147_b200 import sass_mix
+    if rk5 or w.correction_mode != 3 or (w.terms & 32) or not warp_work["warp_steps"]:
+        return None
+    params = 0 if w.uniform else (2 if (w.terms & 16 and len(set(w.beta)) == 1 and len(set(w.chi1)) == 1 and len(set(w.chi2)) == 1) else
+                                  (0 if not (w.terms & 16) and len(set(w.beta)) == 1 and len(set(w.chi1)) == 1 and len(set(w.chi2)) == 1 else 1))
+    mix = sass_mix.analyse(params=params, qm=bool(w.terms & 16))
+    if mix is None:
+        return None
+    g = warp_work["gn_warp_passes"] / warp_work["warp_steps"]
+    per = sass_mix.per_warp_step(mix, g)
+    flop = per["flop"] * 32.0 * warp_work["warp_steps"]              # every lane slot of every executed warp instruction
+    cycles = per["cycles"] * warp_work["warp_steps"] / (4.0 * num_sms)   # per sub-partition, perfectly balanced
+    model_s = cycles / (sm_mhz * 1e6)
+    return {"source": "SASS mix of the built library (paper_1802_00147_b200/sass_mix.py) x mc_get_warp_work",
+            "gn_passes_per_warp_step": g, "fp64_instr_per_warp_step": per["fp64"], "dfma_3_register_per_warp_step": per["dfma_3reg"],
+            "dfma_share_of_fp64_instr": per["DFMA"] / per["fp64"], "executed_flop_per_launch": flop,
+            "executed_tflops": flop / per_launch_s / 1e12,
+            "operand_bandwidth_model": {"cycles_per_warp_step": per["cycles"], "kernel_ms": model_s * 1e3,
+                                        "measured_over_model": per_launch_s / model_s,
+                                        "rule": "3.03 cycles per FMA reading 3 distinct registers, 2.19 with an operand-reuse hit, 2.03 otherwise (mc_fp64_probe)"}}
+
+
 def global_workload(args, world):
     """Config 2 widened to 314*world rows of r0 (same r0 range, same theta axis); the other configs are
     replicated per rank as they are."""
@@ -311,6 +338,7 @@ def run_mc(args):
     info = I.launch_info()
     status = res.status.cpu().numpy()
     fli = res.fli.cpu().numpy() if res.fli is not None else np.zeros(n)
+    warp_work = I.warp_work()                                 # what the warps executed in the last timed launch
     steps_done_per_orbit = res.steps_done.cpu().numpy()
     gn_per_orbit = I.work(n).cpu().numpy()
     steps_done = float(steps_done_per_orbit.sum())            # accepted orbit-steps of one launch (this rank)
@@ -334,6 +362,7 @@ def run_mc(args):
     flop_per_launch = float(alg["flop_per_launch"])
     traj = alg["trajectories_per_orbit"]
     achieved_tf = flop_per_launch / per_launch_s / 1e12
+    executed = executed_from_sass(w, rk5, warp_work, per_launch_s, info["num_sms"], sm_max, value)
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": nominal_tf, "unit": "TFLOP/s",
                 "frac": achieved_tf / nominal_tf,
                 "traffic": NCU_DRAM_BYTES_PER_LAUNCH_314 if (w.name.startswith("config2") and args.grid == 314 and world == 1) else None,
@@ -347,6 +376,7 @@ def run_mc(args):
                 "flop_model": alg["model"], "flop_model_ops": alg["model_ops"],
                 "flop_source": "mc_flop_model: the kernels' math templates run with a counting scalar (tests/test_flop_model.py)",
                 "gn_steps_per_trajectory_step": gn_steps / max(traj * steps_done, 1.0),
+                "executed": executed,
                 "accepted_orbit_steps_per_launch": steps_done, "kernel": "mc::integrate_kernel<%s,QM %s,mode %d>" % ("uniform" if w.uniform else "per-orbit", "on" if w.terms & 16 else "off", w.correction_mode),
                 "kernel_ms_per_launch": dev_ms / args.steps,
                 "regs_per_thread": info["regs_per_thread"], "spill_bytes": info["local_bytes"],

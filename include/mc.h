@@ -194,6 +194,13 @@ int mc_get_dissipation(mc_handle* h, double* out_wg);
  * (0 for the other modes).  Stream-ordered copy.  bench.py derives the algorithmic flop count from it. */
 int mc_get_work(mc_handle* h, int64_t* out_gn_steps);
 
+/* What the warps of the most recent mc_integrate executed, summed over the launch, into HOST int64[2] (synchronises
+ * the stream): [0] passes through the Gauss-Newton loop of mode 3 counted once per WARP (a warp repeats the loop while
+ * any of its 32 lanes needs another step, so this exceeds the per-lane counts of mc_get_work divided by 32 by the
+ * amount of divergence), [1] warp-steps (passes of a warp through the step loop).  bench.py uses both to convert the
+ * SASS instruction mix into executed flop. */
+int mc_get_warp_work(mc_handle* h, int64_t* out_host2);
+
 /* Evaluate pieces of the model on the device with the handle's parameters (used by the parity tests
  * to compare the kernel's fused routines with the oracle one by one).  states: DEVICE double[12][n].
  *   what = 0: out[1][n]  = H                     (eq 1)
@@ -227,6 +234,16 @@ int mc_last_launch_info(mc_handle* h, mc_launch_info* out);
  * `millis` ms; *out_tflops = 2 * FMAs / time (CUDA events).  The roofline denominator of bench.py
  * (MEASURED_PEAKS.json has no FP64 entry).  Synchronous. */
 int mc_fp64_peak(int32_t device, double millis, double* out_tflops, double* out_sm_clock_mhz);
+
+/* Operand bandwidth of the FP64 pipe, measured: a warp-wide FP64 instruction nominally
+ * occupies a sub-partition's 16-lane pipe for 2 cycles, but the register file delivers one 64-bit operand per cycle,
+ * so an FMA that reads three distinct vector registers takes 3.  kind selects the instruction the probe repeats
+ * (8 independent accumulators per thread, 4 warps per sub-partition, about `millis` ms, best of 4):
+ *   0: x <- fma(y, z, x), three distinct registers        2: x <- fma(y, c[bank], x), two registers + constant
+ *   1: x <- fma(y, s, x), s reused by consecutive FMAs    3: x <- x * y (DMUL)
+ * *out_cycles_per_warp_instr = SM cycles (at the device's maximum clock) per warp instruction per sub-partition;
+ * *out_tflops (optional) = the corresponding flop rate of the whole device.  Synchronous.  MC_EINVAL: bad kind. */
+int mc_fp64_probe(int32_t device, double millis, int32_t kind, double* out_cycles_per_warp_instr, double* out_tflops);
 
 /* Algorithmic operation counts of the kernels' own formulation, per trajectory.
  * Host-only, needs no GPU: the library instantiates the math templates the kernels are built from

@@ -17,8 +17,8 @@ MC_OK, MC_EINVAL, MC_ECUDA, MC_EARCH, MC_ENOMEM = 0, -1, -2, -3, -4
 MC_INTEG_RK4, MC_INTEG_RK5 = 0, 1
 
 # every symbol include/mc.h declares (tests/test_abi.py checks the header against this list)
-EXPORTS = ["mc_params_default", "mc_create", "mc_integrate", "mc_integrate_sampled", "mc_integrate_ex", "mc_carry_bytes", "mc_integrate_host", "mc_get_status", "mc_get_work", "mc_get_dissipation", "mc_eval",
-           "mc_last_launch_info", "mc_fp64_peak", "mc_flop_model", "mc_destroy", "mc_strerror"]
+EXPORTS = ["mc_params_default", "mc_create", "mc_integrate", "mc_integrate_sampled", "mc_integrate_ex", "mc_carry_bytes", "mc_integrate_host", "mc_get_status", "mc_get_work", "mc_get_warp_work", "mc_get_dissipation", "mc_eval",
+           "mc_last_launch_info", "mc_fp64_peak", "mc_fp64_probe", "mc_flop_model", "mc_destroy", "mc_strerror"]
 
 
 class MCLibraryError(RuntimeError):
@@ -95,9 +95,11 @@ def load_library():
     lib.mc_get_status.argtypes = [vp, vp, vp]
     lib.mc_get_work.argtypes = [vp, vp]
     lib.mc_get_dissipation.argtypes = [vp, vp]
+    lib.mc_get_warp_work.argtypes = [vp, ctypes.POINTER(ctypes.c_int64)]
     lib.mc_eval.argtypes = [vp, i32, vp, i64, dbl, i32, vp, vp]
     lib.mc_last_launch_info.argtypes = [vp, ctypes.POINTER(mc_launch_info)]
     lib.mc_fp64_peak.argtypes = [i32, dbl, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
+    lib.mc_fp64_probe.argtypes = [i32, dbl, i32, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
     lib.mc_flop_model.argtypes = [ctypes.c_uint32, i32, i32, i32, ctypes.POINTER(mc_flop_model_t)]
     lib.mc_destroy.argtypes = [vp]
     lib.mc_strerror.argtypes = [ctypes.c_int]
@@ -126,6 +128,20 @@ def fp64_peak(device: int = 0, millis: float = 200.0):
     t, c = ctypes.c_double(), ctypes.c_double()
     _check(load_library().mc_fp64_peak(device, millis, ctypes.byref(t), ctypes.byref(c)))
     return t.value, c.value
+
+
+FP64_PROBE_KINDS = {0: "fma(y,z,x): 3 registers", 1: "fma(y,s,x): 2 registers + reused", 2: "fma(y,c[],x): 2 registers + constant",
+                    3: "x*y: DMUL"}
+
+
+def fp64_probe(device: int = 0, millis: float = 100.0) -> dict:
+    """mc_fp64_probe for every kind: {kind name: (cycles per warp instruction per sub-partition, TFLOP/s)}."""
+    out = {}
+    for kind, name in FP64_PROBE_KINDS.items():
+        c, t = ctypes.c_double(), ctypes.c_double()
+        _check(load_library().mc_fp64_probe(device, millis, kind, ctypes.byref(c), ctypes.byref(t)))
+        out[name] = (c.value, t.value)
+    return out
 
 
 def flop_model(terms=TERMS_DEFAULT, correction_mode=3, integrator=0, newton_iters=4) -> dict:
@@ -323,6 +339,12 @@ class Integrator:
         out = torch.empty(n, dtype=torch.int64, device=self.device)
         _check(self._lib.mc_get_work(self._h, out.data_ptr()))
         return out
+
+    def warp_work(self) -> dict:
+        """mc_get_warp_work: Gauss-Newton loop passes counted per warp and warp-steps of the last integrate."""
+        out = (ctypes.c_int64 * 2)()
+        _check(self._lib.mc_get_warp_work(self._h, out))
+        return {"gn_warp_passes": int(out[0]), "warp_steps": int(out[1])}
 
     def dissipation(self, n):
         """mc_get_dissipation: the moving references E0 + W, J0 + G per orbit at the end of the last integrate (handle

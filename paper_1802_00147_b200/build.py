@@ -73,6 +73,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
     subprocess.run([nvcc, "-shared", "-Wno-deprecated-gpu-targets", "-o", LIB + ".tmp"] + [o for o, _ in results] + ["-lcudart_static", "-ldl", "-lrt", "-lpthread"],
                    check=True)
     os.replace(LIB + ".tmp", LIB)
+    try:                                    # SASS instruction mix of the hot loop, for bench.py's `roofline.executed`
+        from . import sass_mix
+        sass_mix.write_json()
+    except Exception as e:                  # cuobjdump missing: bench.py reports executed = null
+        print(f"sass_mix skipped: {e}")
     return LIB
 
 

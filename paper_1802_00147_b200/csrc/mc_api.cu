@@ -141,6 +141,42 @@ dfma_peak_kernel(double* sink, int iters, double a, double b) {
   if (s == 123.456) sink[0] = s;   // never true: keeps the chains alive
 }
 
+// Operand-bandwidth probe (mc_fp64_probe): 8 independent accumulators per thread, x_j <- fma(y_j, *, x_j).
+//   KIND 0: fma(y_j, z_j, x_j) -- three distinct vector registers per instruction
+//   KIND 1: fma(y_j, s,   x_j) -- two + one register shared by consecutive instructions (operand reuse cache)
+//   KIND 2: fma(y_j, c[], x_j) -- two registers + a constant-bank operand
+//   KIND 3: x_j * y_j          -- DMUL, two registers
+__constant__ double g_probe_const[2];
+template <int KIND>
+__global__ void __launch_bounds__(128)
+dfma_operand_probe_kernel(double* sink, int iters, double a, double b) {
+  double x[8], y[8], z[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    x[j] = 1.0 + 1e-9 * (threadIdx.x + j);
+    y[j] = 0.9999999 + 1e-12 * (threadIdx.x + 3 * j) * a;
+    z[j] = 1e-9 * (1 + j) * b + 1e-15 * threadIdx.x;
+  }
+  const double s = a + 1e-15 * threadIdx.x;
+#pragma unroll 1
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int rep = 0; rep < 8; ++rep) {
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        if (KIND == 0) x[j] = fma(y[j], z[j], x[j]);
+        else if (KIND == 1) x[j] = fma(y[j], s, x[j]);
+        else if (KIND == 2) x[j] = fma(y[j], g_probe_const[1], x[j]);
+        else x[j] = x[j] * y[j];
+      }
+    }
+  }
+  double t = 0.0;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) t += x[j] + y[j] + z[j];
+  if (t == 123.456) sink[0] = t + s;   // never true: keeps the chains alive
+}
+
 void fill_args(const mc_handle* h, mc::IntegrateArgs& A) {
   memset(&A, 0, sizeof(A));
   A.beta = h->P.d_beta; A.chi1 = h->P.d_chi1; A.chi2 = h->P.d_chi2; A.kq1 = h->P.d_kq1; A.kq2 = h->P.d_kq2;
@@ -314,10 +350,10 @@ static int integrate_impl(mc_handle* h, const double* states, int64_t n_orbits, 
   A.chunk_len = (int32_t)chunk;
   A.n_chunks = (int32_t)n_chunks;
   A.n_items = A.n_units * n_chunks;
-  rc = h->sched.reserve(16 + sizeof(int32_t) * (size_t)A.n_units);
+  rc = h->sched.reserve(32 + sizeof(int32_t) * (size_t)A.n_units);
   if (rc) return rc;
   A.queue = (unsigned long long*)h->sched.p;
-  A.done = (int32_t*)((char*)h->sched.p + 16);
+  A.done = (int32_t*)((char*)h->sched.p + 32);
   A.resume = resume; A.save_final = user_carry ? 1 : 0;
   if (user_carry) {
     // caller-owned checkpoint (mc_carry_bytes): [17][tp] doubles, [2][tp] u64, [2][tp] int32 -- also the chunk carry
@@ -332,7 +368,7 @@ static int integrate_impl(mc_handle* h, const double* states, int64_t n_orbits, 
     if ((rc = h->carry_g.reserve(sizeof(unsigned long long) * 2 * tp))) return rc;
     A.carry_d = (double*)h->carry_d.p; A.carry_i = (int32_t*)h->carry_i.p; A.carry_g = (unsigned long long*)h->carry_g.p;
   }
-  MC_CUDA(cudaMemsetAsync(h->sched.p, 0, 16 + sizeof(int32_t) * (size_t)A.n_units, h->stream));
+  MC_CUDA(cudaMemsetAsync(h->sched.p, 0, 32 + sizeof(int32_t) * (size_t)A.n_units, h->stream));
   MC_CUDA(fn(h->uc, A, h->num_sms, true, h->stream, &ki));
   h->info.grid = ki.grid;
   h->info.chunk_steps = A.chunk_len;
@@ -365,6 +401,16 @@ int mc_get_work(mc_handle* h, int64_t* out_gn_steps) {
   if (h->last_n == 0) return MC_OK;
   MC_CUDA(cudaSetDevice(h->P.device));
   MC_CUDA(cudaMemcpyAsync(out_gn_steps, h->gn.p, sizeof(int64_t) * (size_t)h->last_n, cudaMemcpyDeviceToDevice, h->stream));
+  return MC_OK;
+}
+
+int mc_get_warp_work(mc_handle* h, int64_t* out_host2) {
+  if (!h || !out_host2) return MC_EINVAL;
+  out_host2[0] = out_host2[1] = 0;
+  if (h->last_n == 0 || !h->sched.p) return MC_OK;
+  MC_CUDA(cudaSetDevice(h->P.device));
+  MC_CUDA(cudaMemcpyAsync(out_host2, (char*)h->sched.p + 8, 2 * sizeof(int64_t), cudaMemcpyDeviceToHost, h->stream));
+  MC_CUDA(cudaStreamSynchronize(h->stream));
   return MC_OK;
 }
 
@@ -462,6 +508,49 @@ int mc_fp64_peak(int32_t device, double millis, double* out_tflops, double* out_
   if (out_sm_clock_mhz) {
     // cycles per second implied by one DFMA per lane per clock on 64 lanes per SM
     *out_sm_clock_mhz = best * 1e12 / (2.0 * 64.0 * prop.multiProcessorCount) / 1e6;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(sink);
+  return MC_OK;
+}
+
+int mc_fp64_probe(int32_t device, double millis, int32_t kind, double* out_cycles_per_warp_instr, double* out_tflops) {
+  if (!out_cycles_per_warp_instr || !(millis > 0.0) || kind < 0 || kind > 3) return MC_EINVAL;
+  MC_CUDA(cudaSetDevice(device));
+  cudaDeviceProp prop;
+  MC_CUDA(cudaGetDeviceProperties(&prop, device));
+  const double hc[2] = {0.0, 0.999999999};
+  MC_CUDA(cudaMemcpyToSymbol(g_probe_const, hc, sizeof(hc)));
+  double* sink = nullptr;
+  MC_CUDA(cudaMalloc(&sink, sizeof(double)));
+  cudaEvent_t e0, e1;
+  MC_CUDA(cudaEventCreate(&e0));
+  MC_CUDA(cudaEventCreate(&e1));
+  const int warps_per_smsp = 4, block = 128, grid = prop.multiProcessorCount * warps_per_smsp;   // one warp per sub-partition per block
+  int iters = 2000;
+  float ms = 0.f, best = 1e30f;
+  for (int pass = 0; pass < 6; ++pass) {
+    MC_CUDA(cudaEventRecord(e0, 0));
+    switch (kind) {
+      case 0: dfma_operand_probe_kernel<0><<<grid, block>>>(sink, iters, 0.999999999, 1e-9); break;
+      case 1: dfma_operand_probe_kernel<1><<<grid, block>>>(sink, iters, 0.999999999, 1e-9); break;
+      case 2: dfma_operand_probe_kernel<2><<<grid, block>>>(sink, iters, 0.999999999, 1e-9); break;
+      default: dfma_operand_probe_kernel<3><<<grid, block>>>(sink, iters, 0.999999999, 1e-9); break;
+    }
+    MC_CUDA(cudaEventRecord(e1, 0));
+    MC_CUDA(cudaEventSynchronize(e1));
+    MC_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    if (pass >= 2 && ms < best) best = ms;
+    if (pass < 2 && ms > 0.f) iters = (int)fmin(2.0e6, fmax(100.0, iters * millis / ms));
+  }
+  // warp instructions per sub-partition = iters * 64 * warps_per_smsp; cycles at the device's maximum SM clock
+  const double inst = (double)iters * 64.0 * warps_per_smsp;
+  const double clk = prop.clockRate * 1e3;
+  *out_cycles_per_warp_instr = best * 1e-3 * clk / inst;
+  if (out_tflops) {
+    const double flop_per_inst = kind == 3 ? 1.0 : 2.0;
+    *out_tflops = flop_per_inst * 32.0 * inst * 4.0 * prop.multiProcessorCount / (best * 1e-3) / 1e12;
   }
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);

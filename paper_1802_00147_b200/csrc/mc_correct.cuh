@@ -29,17 +29,20 @@ MC_DEV void references(const C& c, const T* z, RefsT<T>& R) {
 // Iteration control (R6): a lane repeats the step until its last update
 // satisfies |(dr,dp)|^2 <= tol^2 p.p, at most `iters` times.  The decision is per lane (results do not
 // depend on the neighbours); the warp leaves the loop when no lane needs another step.  Must be called
-// by all 32 lanes.  Returns the number of steps this lane took.
+// by all 32 lanes.  Returns the number of steps this lane took; warp_passes receives the number of passes the WARP
+// made through the loop body (= the largest step count among its lanes: what the pipe really executed).
 template <bool QM, class C, class T>
-MC_DEV int project_six(const C& c, T* z, const RefsT<T>& R, int iters, double tol2) {
+MC_DEV int project_six(const C& c, T* z, const RefsT<T>& R, int iters, double tol2, int& warp_passes) {
   T Lt[3];
 #pragma unroll
   for (int i = 0; i < 3; ++i) Lt[i] = fma(-c[K_S2], z[9 + i], fma(-c[K_S1], z[6 + i], R.J0[i]));
   bool need = true;
   int done = 0;
+  warp_passes = 0;
 #pragma unroll 1
   for (int it = 0; it < iters; ++it) {
     if (!warp_any(need)) break;
+    ++warp_passes;
     if (need) {
       T g[12], H;
       pn_eval<QM, false, true, false>(c, z, g, H);
@@ -155,13 +158,21 @@ MC_DEV bool dual_scaling(const C& c, T* z, const RefsT<T>& R, int iters, double 
 }
 
 // C_mode: spins first (eq 10), then (r,p) with the corrected spins.
-// gn_steps receives the number of Gauss-Newton steps mode 3 took (0 otherwise).
+// gn_steps receives the number of Gauss-Newton steps mode 3 took (0 otherwise), warp_passes the passes of the warp.
+template <int MODE, bool QM, class C, class T>
+MC_DEV bool correct(const C& c, T* z, const RefsT<T>& R, int iters, double tol, int& gn_steps, int& warp_passes);
 template <int MODE, bool QM, class C, class T>
 MC_DEV bool correct(const C& c, T* z, const RefsT<T>& R, int iters, double tol, int& gn_steps) {
+  int wp;
+  return correct<MODE, QM>(c, z, R, iters, tol, gn_steps, wp);
+}
+template <int MODE, bool QM, class C, class T>
+MC_DEV bool correct(const C& c, T* z, const RefsT<T>& R, int iters, double tol, int& gn_steps, int& warp_passes) {
   gn_steps = 0;
+  warp_passes = 0;
   if (MODE >= 1) { normalise3(z + 6); normalise3(z + 9); }
   if (MODE == 2) return dual_scaling<QM>(c, z, R, iters, tol);
-  if (MODE == 3) gn_steps = project_six<QM>(c, z, R, iters, tol * tol);
+  if (MODE == 3) gn_steps = project_six<QM>(c, z, R, iters, tol * tol, warp_passes);
   return true;
 }
 

@@ -40,7 +40,7 @@ struct IntegrateArgs {
   double* samples;            // [n_steps / sample_interval][12][n] or null: orbit states after steps interval, 2 interval, ...
   int32_t sample_interval;
   // scheduling
-  unsigned long long* queue;  // [0] = next item
+  unsigned long long* queue;  // [0] = next item; [1] += Gauss-Newton passes of the warps; [2] += warp-steps executed (mc_get_warp_work)
   int32_t* done;              // [n_units] chunks completed per unit
   double* carry_d;            // [17][n_traj_padded]: y[12], E0, J0[3] (MC_TERM_RR: E0 + W, J0 + G), acc
   double* out_diss;           // [4][n]: E0 + W, J0 + G of the orbit at the end (MC_TERM_RR), handle-owned
@@ -139,6 +139,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
     // earlier chunks / earlier calls stay in the carry buffer and are added when the item is parked or stored
     int steps = 0;
     unsigned gn_chunk = 0;
+    unsigned gn_warp = 0, warp_steps = 0;  // passes of this WARP through the Gauss-Newton loop / the step loop (work accounting)
     double acc = 0.0;
     int until_renorm = A.renorm_interval;
 
@@ -204,17 +205,19 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
         }
         break;
       }
+      ++warp_steps;
       double z[NS];
       base_step<INTEG, QM, RR>(c, y, A.h, z);
-      int gn;
+      int gn, gnw;
       bool ok;
       if constexpr (RR) {   // the manifold has moved by the work and torque of the step (integral invariant relation)
         Refs Rm;
         Rm.E0 = z[12]; Rm.J0[0] = z[13]; Rm.J0[1] = z[14]; Rm.J0[2] = z[15];
-        ok = correct<MODE, QM>(c, z, Rm, A.newton_iters, A.newton_tol, gn);
+        ok = correct<MODE, QM>(c, z, Rm, A.newton_iters, A.newton_tol, gn, gnw);
       } else {
-        ok = correct<MODE, QM>(c, z, R, A.newton_iters, A.newton_tol, gn);
+        ok = correct<MODE, QM>(c, z, R, A.newton_iters, A.newton_tol, gn, gnw);
       }
+      gn_warp += (unsigned)gnw;
       if (MODE == 2 && !ok && !role_shadow && !frozen) flag = ST_NEWTON_FLAG;
       // status of the completed step (R13): non-finite anywhere in the pair, else |r| of the main
       int code = ST_OK;
@@ -276,6 +279,10 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
       }
     }
 
+    if (lane == 0) {   // what the pipe executed, per launch (mc_get_warp_work)
+      atomicAdd(A.queue + 1, (unsigned long long)gn_warp);
+      atomicAdd(A.queue + 2, (unsigned long long)warp_steps);
+    }
     const bool last = chunk + 1 == A.n_chunks;
     const bool carried = chunk > 0 || A.resume;
     unsigned long long gn_total = gn_chunk;

@@ -34,7 +34,7 @@ UNIT = "orbit-steps/s"
 # dram__bytes_read.sum + dram__bytes_write.sum from the ncu capture of that very launch configuration
 # (profiles/r02_ncu_traffic_full_launch.md).  Outputs (31 MB) and the carry buffer (31 MB) live in the 126 MB L2;
 # algorithmic: 340 B per orbit.
-NCU_DRAM_BYTES_PER_LAUNCH_314 = None   # set below once the round-2 capture exists
+NCU_DRAM_BYTES_PER_LAUNCH_314 = 10129920 + 7862528   # read + write, bytes
 FP64_LANES_PER_SM = 64
 
 
@@ -366,7 +366,8 @@ def run_mc(args):
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": nominal_tf, "unit": "TFLOP/s",
                 "frac": achieved_tf / nominal_tf,
                 "traffic": NCU_DRAM_BYTES_PER_LAUNCH_314 if (w.name.startswith("config2") and args.grid == 314 and world == 1) else None,
-                "traffic_unit": "bytes per launch (ncu capture of a 4000-step launch, profiles/r01c_ncu_integrate_kernel_mode3.md)",
+                "traffic_unit": "bytes per launch: dram__bytes_read.sum + dram__bytes_write.sum of one full-length (1e5-step) launch of "
+                                "this kernel and grid under ncu (profiles/r02_ncu_integrate_kernel_mode3.md); not re-measured in this run",
                 "algorithmic_bytes_per_launch": 340.0 * n,
                 "peak_source": f"derived: {info['num_sms']} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x {sm_max:.0f} MHz "
                                "(MEASURED_PEAKS.json has no FP64 entry)",
@@ -377,7 +378,10 @@ def run_mc(args):
                 "flop_source": "mc_flop_model: the kernels' math templates run with a counting scalar (tests/test_flop_model.py)",
                 "gn_steps_per_trajectory_step": gn_steps / max(traj * steps_done, 1.0),
                 "executed": executed,
-                "accepted_orbit_steps_per_launch": steps_done, "kernel": "mc::integrate_kernel<%s,QM %s,mode %d>" % ("uniform" if w.uniform else "per-orbit", "on" if w.terms & 16 else "off", w.correction_mode),
+                "accepted_orbit_steps_per_launch": steps_done, "kernel": "mc::integrate_kernel<%s,QM %s,mode %d,%s%s>" % (
+                    "per-orbit" if info["variant"] & 1 else ("per-orbit kappa" if info["variant"] & 4 else "uniform"),
+                    "on" if info["variant"] & 2 else "off", (info["variant"] >> 4) & 3, "RK5" if info["variant"] & 256 else "RK4",
+                    ",2.5PN" if info["variant"] & 8 else ""),
                 "kernel_ms_per_launch": dev_ms / args.steps,
                 "regs_per_thread": info["regs_per_thread"], "spill_bytes": info["local_bytes"],
                 "blocks_per_sm": info["blocks_per_sm"], "grid": info["grid"], "block": info["block"]}

@@ -26,11 +26,69 @@ MC_DEV void references(const C& c, const T* z, RefsT<T>& R) {
 // M^-1 is closed-form (Woodbury): M^-1 x = N(x)/D, D = (r.r + p.p) |L|^2,
 //   N(x) = |L|^2 x + r (rr (r.x) + rp (p.x)) + p (rp (r.x) + pp (p.x)),
 // so the 4x4 solve needs one reciprocal.  The oracle solves the same system by pivoted elimination.
-// Iteration control (R6): a lane repeats the step until its last update
-// satisfies |(dr,dp)|^2 <= tol^2 p.p, at most `iters` times.  The decision is per lane (results do not
-// depend on the neighbours); the warp leaves the loop when no lane needs another step.  Must be called
-// by all 32 lanes.  Returns the number of steps this lane took; warp_passes receives the number of passes the WARP
-// made through the loop body (= the largest step count among its lanes: what the pipe really executed).
+//
+// gn_pass: ONE Gauss-Newton step on (r, p) = z[0:6] with the spins z[6:12] held fixed, towards energy E0 and orbital
+// angular momentum Lt = J0 - S1 - S2.  Returns whether another step is needed: |(dr,dp)|^2 > tol^2 p.p (R6;
+// PAPER.md:146, 197); false also for a non-finite step.
+template <bool QM, class C, class T>
+MC_DEV bool gn_pass(const C& c, T* z, const T& E0, const T* Lt, double tol2) {
+  T g[12], H;
+  pn_eval<QM, false, true, false>(c, z, g, H);
+  T* r = z;
+  T* p = z + 3;
+  const T* a = g;
+  const T* b = g + 3;
+  T fL[3], cv[3];
+  cross3(r, p, fL);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) fL[i] -= Lt[i];
+  const T f0 = H - E0;
+  // c = a x p + r x b
+  cv[0] = fma(r[1], b[2], fma(-r[2], b[1], fma(a[1], p[2], -(a[2] * p[1]))));
+  cv[1] = fma(r[2], b[0], fma(-r[0], b[2], fma(a[2], p[0], -(a[0] * p[2]))));
+  cv[2] = fma(r[0], b[1], fma(-r[1], b[0], fma(a[0], p[1], -(a[1] * p[0]))));
+  const T gg = dot3(a, a) + dot3(b, b);
+  const T rr = dot3(r, r), pp = dot3(p, p), rp = dot3(r, p);
+  const T LL = fma(rr, pp, -(rp * rp));
+  const T D = (rr + pp) * LL;
+  // N(c), N(fL)
+  const T rc = dot3(r, cv), pc = dot3(p, cv), rf = dot3(r, fL), pf = dot3(p, fL);
+  const T cr_ = fma(rp, pc, rr * rc), cp_ = fma(pp, pc, rp * rc);
+  const T fr_ = fma(rp, pf, rr * rf), fp_ = fma(pp, pf, rp * rf);
+  T Nc[3], Nf[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    Nc[i] = fma(p[i], cp_, fma(r[i], cr_, LL * cv[i]));
+    Nf[i] = fma(p[i], fp_, fma(r[i], fr_, LL * fL[i]));
+  }
+  const T S = fma(gg, D, -dot3(cv, Nc));
+  const T num = fma(D, f0, -dot3(cv, Nf));
+  const T DS = D * S;
+  const T inv = (DS != 0.0) ? rcp_nz(DS) : T(0.0);      // singular only for r || p or a circular orbit
+  const T l0 = num * D * inv;                         // num / S
+  const T sD = S * inv;                               // 1 / D
+  T lL[3], d1[3], d2[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) lL[i] = fma(-l0, Nc[i], Nf[i]) * sD;
+  cross3(p, lL, d1);   // dr = l0 a + p x lL
+  cross3(lL, r, d2);   // dp = l0 b + lL x r
+  T dd = 0.0;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    const T dr = fma(l0, a[i], d1[i]);
+    const T dp = fma(l0, b[i], d2[i]);
+    dd = fma(dr, dr, fma(dp, dp, dd));
+    r[i] -= dr;
+    p[i] -= dp;
+  }
+  return dd > tol2 * pp;
+}
+
+// Iteration control (R6): a lane repeats the step until its last update satisfies the test, at most `iters`
+// times.  The decision is per lane (results do not depend on the neighbours); the warp leaves the loop when no lane
+// needs another step.  Must be called by all 32 lanes.  Returns the number of steps this lane took; warp_passes
+// receives the number of passes the WARP made through the loop body (= the largest step count among its lanes: what
+// the pipe really executed).
 template <bool QM, class C, class T>
 MC_DEV int project_six(const C& c, T* z, const RefsT<T>& R, int iters, double tol2, int& warp_passes) {
   T Lt[3];
@@ -44,57 +102,8 @@ MC_DEV int project_six(const C& c, T* z, const RefsT<T>& R, int iters, double to
     if (!warp_any(need)) break;
     ++warp_passes;
     if (need) {
-      T g[12], H;
-      pn_eval<QM, false, true, false>(c, z, g, H);
-      T* r = z;
-      T* p = z + 3;
-      const T* a = g;
-      const T* b = g + 3;
-      T fL[3], cv[3];
-      cross3(r, p, fL);
-#pragma unroll
-      for (int i = 0; i < 3; ++i) fL[i] -= Lt[i];
-      const T f0 = H - R.E0;
-      // c = a x p + r x b
-      cv[0] = fma(r[1], b[2], fma(-r[2], b[1], fma(a[1], p[2], -(a[2] * p[1]))));
-      cv[1] = fma(r[2], b[0], fma(-r[0], b[2], fma(a[2], p[0], -(a[0] * p[2]))));
-      cv[2] = fma(r[0], b[1], fma(-r[1], b[0], fma(a[0], p[1], -(a[1] * p[0]))));
-      const T gg = dot3(a, a) + dot3(b, b);
-      const T rr = dot3(r, r), pp = dot3(p, p), rp = dot3(r, p);
-      const T LL = fma(rr, pp, -(rp * rp));
-      const T D = (rr + pp) * LL;
-      // N(c), N(fL)
-      const T rc = dot3(r, cv), pc = dot3(p, cv), rf = dot3(r, fL), pf = dot3(p, fL);
-      const T cr_ = fma(rp, pc, rr * rc), cp_ = fma(pp, pc, rp * rc);
-      const T fr_ = fma(rp, pf, rr * rf), fp_ = fma(pp, pf, rp * rf);
-      T Nc[3], Nf[3];
-#pragma unroll
-      for (int i = 0; i < 3; ++i) {
-        Nc[i] = fma(p[i], cp_, fma(r[i], cr_, LL * cv[i]));
-        Nf[i] = fma(p[i], fp_, fma(r[i], fr_, LL * fL[i]));
-      }
-      const T S = fma(gg, D, -dot3(cv, Nc));
-      const T num = fma(D, f0, -dot3(cv, Nf));
-      const T DS = D * S;
-      const T inv = (DS != 0.0) ? rcp_nz(DS) : T(0.0);      // singular only for r || p or a circular orbit
-      const T l0 = num * D * inv;                         // num / S
-      const T sD = S * inv;                               // 1 / D
-      T lL[3], d1[3], d2[3];
-#pragma unroll
-      for (int i = 0; i < 3; ++i) lL[i] = fma(-l0, Nc[i], Nf[i]) * sD;
-      cross3(p, lL, d1);   // dr = l0 a + p x lL
-      cross3(lL, r, d2);   // dp = l0 b + lL x r
-      T dd = 0.0;
-#pragma unroll
-      for (int i = 0; i < 3; ++i) {
-        const T dr = fma(l0, a[i], d1[i]);
-        const T dp = fma(l0, b[i], d2[i]);
-        dd = fma(dr, dr, fma(dp, dp, dd));
-        r[i] -= dr;
-        p[i] -= dp;
-      }
+      need = gn_pass<QM>(c, z, R.E0, Lt, tol2);
       ++done;
-      need = dd > tol2 * pp;       // false also for a non-finite step
     }
   }
   return done;

@@ -950,3 +950,40 @@ def test_papers_dissipative_orbit3_at_full_length(mc, integ):
     assert (np.abs(I1[0] - ref[0]) / np.abs(ginv[0])).max() <= DRIFT_TOL
     assert (np.linalg.norm(I1[1:4] - ref[1:4], axis=0) / np.linalg.norm(ginv[1:4], axis=0)).max() <= DRIFT_TOL
     assert (gfli < FLI_THRESHOLD).all() and (o.fli < FLI_THRESHOLD).all() and np.abs(gfli - o.fli).max() < 0.1
+
+
+@pytest.mark.parametrize("variant", ["kappa-qm", "rr", "rr-kappa-qm-rk5"])
+def test_edge_cases_of_the_round2_kernel_variants(mc, variant):
+    """Empty and ragged batches, n_steps = 0, in-place output and orbit permutation for the kernel variants added in round 2
+    (per-orbit kappa, 2.5PN): the same properties test_edge_cases / test_batch_properties check for the base kernel."""
+    w = workloads.config3(n_r=7, n_theta=19, qm=True)                       # 133 orbits: ragged (4 blocks + 10 lanes)
+    kw = {k: v for k, v in w.params().items() if k != "terms"}
+    terms = {"kappa-qm": w.terms, "rr": 15 | RR, "rr-kappa-qm-rk5": w.terms | RR}[variant]
+    if variant == "rr":
+        kw = dict(beta=0.8, chi1=0.9, chi2=0.9)
+    integ = mc.MC_INTEG_RK5 if variant.endswith("rk5") else mc.MC_INTEG_RK4
+    n = w.n_orbits
+
+    def sub(idx):
+        return {k: (v[idx] if hasattr(v, "__len__") else v) for k, v in kw.items()}
+    with mc.Integrator(terms=terms, integrator=integ, **kw) as I:
+        e = I.integrate(w.states[:, :0], 1.0, 10, 3, shadow_eps=1e-8)
+        assert e.states.shape == (12, 0)
+        zero = I.integrate(w.states, 1.0, 0, 3, shadow_eps=1e-8)
+        assert np.allclose(zero.states.cpu().numpy(), w.states, rtol=1e-15, atol=0) and (zero.steps_done.cpu().numpy() == 0).all()
+        a = I.integrate(w.states, 1.0, 400, 3, shadow_eps=1e-8)
+        A, Af = a.states.cpu().numpy(), a.fli.cpu().numpy()
+        zt = torch.as_tensor(w.states, device="cuda").clone()
+        c = I.integrate(zt, 1.0, 400, 3, shadow_eps=1e-8, out_states=zt)             # in place
+        assert np.array_equal(c.states.cpu().numpy(), A)
+        if terms & RR:
+            ref = I.dissipation(n).cpu().numpy()
+            assert (ref[0] < a.invariants.cpu().numpy()[0])[a.status.cpu().numpy() == 0].all()      # energy only goes down
+    perm = np.random.default_rng(4).permutation(n)
+    with mc.Integrator(terms=terms, integrator=integ, **sub(perm)) as I:
+        b = I.integrate(w.states[:, perm], 1.0, 400, 3, shadow_eps=1e-8)
+    assert np.array_equal(A[:, perm], b.states.cpu().numpy(), equal_nan=True)         # orbits are independent
+    assert np.array_equal(Af[perm], b.fli.cpu().numpy(), equal_nan=True)
+    with mc.Integrator(terms=terms, integrator=integ, **sub(np.arange(1))) as I:     # a single orbit
+        one = I.integrate(w.states[:, :1], 1.0, 400, 3, shadow_eps=1e-8)
+    assert np.array_equal(one.states.cpu().numpy()[:, 0], A[:, 0], equal_nan=True)

@@ -201,6 +201,13 @@ int mc_get_work(mc_handle* h, int64_t* out_gn_steps);
  * SASS instruction mix into executed flop. */
 int mc_get_warp_work(mc_handle* h, int64_t* out_host2);
 
+/* Checked build only (libmc_checked.so, compiled with -DMC_CHECKED by paper_1802_00147_b200/build.py): the integration
+ * kernel tests every index and pointer before the global access that uses it; *out_line (HOST) = 0 if no test of the most
+ * recent mc_integrate failed, else the source line (csrc/mc_kernel.cuh) of the first one that did.  Synchronises the
+ * stream.  The product library compiles the tests away and reports -1.  (compute-sanitizer is closed on this GPU pool;
+ * the GPU tests run a representative set of launches through the checked library instead.) */
+int mc_debug_check(mc_handle* h, int64_t* out_line);
+
 /* Evaluate pieces of the model on the device with the handle's parameters (used by the parity tests
  * to compare the kernel's fused routines with the oracle one by one).  states: DEVICE double[12][n].
  *   what = 0: out[1][n]  = H                     (eq 1)

@@ -17,7 +17,7 @@ MC_OK, MC_EINVAL, MC_ECUDA, MC_EARCH, MC_ENOMEM = 0, -1, -2, -3, -4
 MC_INTEG_RK4, MC_INTEG_RK5 = 0, 1
 
 # every symbol include/mc.h declares (tests/test_abi.py checks the header against this list)
-EXPORTS = ["mc_params_default", "mc_create", "mc_integrate", "mc_integrate_sampled", "mc_integrate_ex", "mc_carry_bytes", "mc_integrate_host", "mc_get_status", "mc_get_work", "mc_get_warp_work", "mc_get_dissipation", "mc_eval",
+EXPORTS = ["mc_params_default", "mc_create", "mc_integrate", "mc_integrate_sampled", "mc_integrate_ex", "mc_carry_bytes", "mc_integrate_host", "mc_get_status", "mc_get_work", "mc_get_warp_work", "mc_get_dissipation", "mc_debug_check", "mc_eval",
            "mc_last_launch_info", "mc_fp64_peak", "mc_fp64_probe", "mc_flop_model", "mc_destroy", "mc_strerror"]
 
 
@@ -96,6 +96,7 @@ def load_library():
     lib.mc_get_work.argtypes = [vp, vp]
     lib.mc_get_dissipation.argtypes = [vp, vp]
     lib.mc_get_warp_work.argtypes = [vp, ctypes.POINTER(ctypes.c_int64)]
+    lib.mc_debug_check.argtypes = [vp, ctypes.POINTER(ctypes.c_int64)]
     lib.mc_eval.argtypes = [vp, i32, vp, i64, dbl, i32, vp, vp]
     lib.mc_last_launch_info.argtypes = [vp, ctypes.POINTER(mc_launch_info)]
     lib.mc_fp64_peak.argtypes = [i32, dbl, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
@@ -345,6 +346,12 @@ class Integrator:
         out = (ctypes.c_int64 * 2)()
         _check(self._lib.mc_get_warp_work(self._h, out))
         return {"gn_warp_passes": int(out[0]), "warp_steps": int(out[1])}
+
+    def debug_check(self) -> int:
+        """mc_debug_check: -1 for the product library; checked build: 0 = clean, else the source line of the failed test."""
+        out = ctypes.c_int64()
+        _check(self._lib.mc_debug_check(self._h, ctypes.byref(out)))
+        return int(out.value)
 
     def dissipation(self, n):
         """mc_get_dissipation: the moving references E0 + W, J0 + G per orbit at the end of the last integrate (handle

@@ -8,6 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libmc.so")
+LIB_CHECKED = os.path.join(HERE, "libmc_checked.so")     # -DMC_CHECKED: index / pointer tests before every global access
 SOURCES = ["mc_api.cu", "mc_kernel_mode0.cu", "mc_kernel_mode1.cu", "mc_kernel_mode2.cu", "mc_kernel_mode3.cu",
            "mc_flop_model.cpp"]       # .cpp: host-only C++ (the flop model), compiled by nvcc's host compiler
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
@@ -46,15 +47,25 @@ def spill_report(log: str):
     return bad
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not is_stale():
+def build_checked(force: bool = False) -> str:
+    """libmc_checked.so: the same sources with -DMC_CHECKED (mc_debug_check).  Used by the GPU tests only."""
+    if not force and os.path.exists(LIB_CHECKED) and not any(os.path.getmtime(f) > os.path.getmtime(LIB_CHECKED) for f in _deps()):
+        return LIB_CHECKED
+    return build(force=True, checked=True)
+
+
+def build(force: bool = False, verbose: bool = False, checked: bool = False) -> str:
+    if not checked and not force and not is_stale():
         return LIB
-    os.makedirs(OBJ, exist_ok=True)
+    obj_dir = OBJ + ("_checked" if checked else "")
+    lib = LIB_CHECKED if checked else LIB
+    flags = NVCC_FLAGS + (["-DMC_CHECKED"] if checked else [])
+    os.makedirs(obj_dir, exist_ok=True)
     nvcc = os.environ.get("NVCC", "nvcc")
 
     def compile_one(src):
-        obj = os.path.join(OBJ, os.path.splitext(src)[0] + ".o")
-        r = subprocess.run([nvcc] + NVCC_FLAGS + ["-c", os.path.join(CSRC, src), "-o", obj],
+        obj = os.path.join(obj_dir, os.path.splitext(src)[0] + ".o")
+        r = subprocess.run([nvcc] + flags + ["-c", os.path.join(CSRC, src), "-o", obj],
                            capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError(f"nvcc failed on {src}:\n{r.stdout}\n{r.stderr}")
@@ -63,16 +74,18 @@ def build(force: bool = False, verbose: bool = False) -> str:
     with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
         results = list(ex.map(compile_one, SOURCES))
     log = "".join(err for _, err in results)
-    with open(os.path.join(OBJ, "ptxas.log"), "w") as f:
+    with open(os.path.join(obj_dir, "ptxas.log"), "w") as f:
         f.write(log)
     if verbose:
         print(log)
     bad = spill_report(log)
-    if bad:
+    if bad and not checked:                 # the checked build is a debugging aid: spills there are tolerated
         raise RuntimeError("register spills (north_star demands none):\n" + "\n".join(f"{k}: {l}" for k, l in bad))
-    subprocess.run([nvcc, "-shared", "-Wno-deprecated-gpu-targets", "-o", LIB + ".tmp"] + [o for o, _ in results] + ["-lcudart_static", "-ldl", "-lrt", "-lpthread"],
+    subprocess.run([nvcc, "-shared", "-Wno-deprecated-gpu-targets", "-o", lib + ".tmp"] + [o for o, _ in results] + ["-lcudart_static", "-ldl", "-lrt", "-lpthread"],
                    check=True)
-    os.replace(LIB + ".tmp", LIB)
+    os.replace(lib + ".tmp", lib)
+    if checked:
+        return lib
     try:                                    # SASS instruction mix of the hot loop, for bench.py's `roofline.executed`
         from . import sass_mix
         sass_mix.write_json()

@@ -414,6 +414,21 @@ int mc_get_warp_work(mc_handle* h, int64_t* out_host2) {
   return MC_OK;
 }
 
+int mc_debug_check(mc_handle* h, int64_t* out_line) {
+  if (!h || !out_line) return MC_EINVAL;
+#ifndef MC_CHECKED
+  *out_line = -1;
+  return MC_OK;
+#else
+  *out_line = 0;
+  if (h->last_n == 0 || !h->sched.p) return MC_OK;
+  MC_CUDA(cudaSetDevice(h->P.device));
+  MC_CUDA(cudaMemcpyAsync(out_line, (char*)h->sched.p + 24, sizeof(int64_t), cudaMemcpyDeviceToHost, h->stream));
+  MC_CUDA(cudaStreamSynchronize(h->stream));
+  return MC_OK;
+#endif
+}
+
 int mc_get_dissipation(mc_handle* h, double* out_wg) {
   if (!h || !out_wg) return MC_EINVAL;
   if (!(h->P.terms & MC_TERM_RR)) return MC_EINVAL;

@@ -57,6 +57,15 @@ struct IntegrateArgs {
 
 enum { ST_OK = 0, ST_MERGED = 1, ST_UNBOUND = 2, ST_NONFINITE = 3, ST_NEWTON_FLAG = 256 };
 
+// Checked build (-DMC_CHECKED, libmc_checked.so; compute-sanitizer is closed on this GPU pool): every index and pointer
+// the kernel is about to use for a global access is tested first; the source line of the first failed test lands in
+// queue[3] (mc_debug_check).  The product build compiles the tests away.
+#ifdef MC_CHECKED
+#define MC_CHK(cond) do { if (!(cond)) atomicCAS(A.queue + 3, 0ULL, (unsigned long long)__LINE__); } while (0)
+#else
+#define MC_CHK(cond) do { } while (0)
+#endif
+
 #ifndef MC_BLOCK
 #define MC_BLOCK 128
 #endif
@@ -127,6 +136,10 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
     const bool role_shadow = shadow && (t & 1);
     const bool active = orbit_raw < A.n;
     const int64_t orbit = active ? orbit_raw : (A.n - 1);   // idle lanes shadow-compute a valid orbit, never store
+    MC_CHK(unit >= 0 && unit < A.n_units && chunk >= 0 && chunk < A.n_chunks);
+    MC_CHK(t >= 0 && t < tp && orbit >= 0 && orbit < A.n);
+    MC_CHK(PARAMS == PARAMS_UNIFORM || (A.kq1 != nullptr && A.kq2 != nullptr));
+    MC_CHK(PARAMS != PARAMS_PER_ORBIT || (A.beta != nullptr && A.chi1 != nullptr && A.chi2 != nullptr));
 
     using CP = typename ConstsOf<PARAMS>::type;
     const CP c = make_consts<PARAMS, CP>(uc, A, orbit, smem);
@@ -145,6 +158,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
 
     if (chunk == 0 && !A.resume) {
       // prologue: coalesced SoA load, eq (10) on the input, reference integrals
+      MC_CHK(A.states != nullptr);
 #pragma unroll
       for (int i = 0; i < 12; ++i) y[i] = A.states[(int64_t)i * A.n + orbit];
       if (MODE >= 1) { normalise3(y + 6); normalise3(y + 9); }
@@ -175,6 +189,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
       }
       __syncwarp();
       __threadfence();
+      MC_CHK(A.carry_d != nullptr && A.carry_i != nullptr && A.carry_g != nullptr && A.done != nullptr);
 #pragma unroll
       for (int i = 0; i < 12; ++i) y[i] = __ldcg(A.carry_d + (int64_t)i * tp + t);   // L2 only: L1 may be stale
       R.E0 = __ldcg(A.carry_d + 12 * tp + t);
@@ -198,6 +213,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
         if (A.samples != nullptr && !role_shadow && active) {      // whole warp dropped: remaining samples of this chunk
           for (int kk = k; kk < k_end; ++kk)
             if ((kk + 1) % A.sample_interval == 0) {
+              MC_CHK((kk + 1) / A.sample_interval >= 1 && (kk + 1) / A.sample_interval <= A.n_steps / A.sample_interval);
               double* dst = A.samples + ((int64_t)((kk + 1) / A.sample_interval - 1) * 12) * A.n + orbit;
 #pragma unroll
               for (int i = 0; i < 12; ++i) __stcs(dst + (int64_t)i * A.n, y[i]);
@@ -245,6 +261,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
         // sampled output: the orbit's current state, its frozen state once it has been dropped
         until_sample = A.sample_interval;
         if (!role_shadow && active) {
+          MC_CHK(A.samples != nullptr && (k + 1) / A.sample_interval >= 1 && (k + 1) / A.sample_interval <= A.n_steps / A.sample_interval);
           double* dst = A.samples + ((int64_t)((k + 1) / A.sample_interval - 1) * 12) * A.n + orbit;
 #pragma unroll
           for (int i = 0; i < 12; ++i) __stcs(dst + (int64_t)i * A.n, y[i]);
@@ -293,6 +310,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
     }
     if (!last || A.save_final) {
       // park the state in the carry buffer (and publish the chunk unless it is the last)
+      MC_CHK(A.carry_d != nullptr && A.carry_i != nullptr && A.carry_g != nullptr && A.done != nullptr);
 #pragma unroll
       for (int i = 0; i < 12; ++i) __stcg(A.carry_d + (int64_t)i * tp + t, y[i]);
       if constexpr (RR) { R.E0 = y[12]; R.J0[0] = y[13]; R.J0[1] = y[14]; R.J0[2] = y[15]; }
@@ -314,6 +332,9 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
     }
 
     // epilogue: FLI from the final separation, invariants, coalesced SoA stores
+    MC_CHK(A.out_states != nullptr && A.out_status != nullptr && A.out_step != nullptr && A.out_gn != nullptr);
+    MC_CHK(!shadow || A.out_fli != nullptr);
+    MC_CHK(!RR || A.out_diss != nullptr);
     if (shadow) gn_total += __shfl_xor_sync(0xffffffffu, gn_total, 1);
     if (shadow) {
       double ym[12];

@@ -987,3 +987,23 @@ def test_edge_cases_of_the_round2_kernel_variants(mc, variant):
     with mc.Integrator(terms=terms, integrator=integ, **sub(np.arange(1))) as I:     # a single orbit
         one = I.integrate(w.states[:, :1], 1.0, 400, 3, shadow_eps=1e-8)
     assert np.array_equal(one.states.cpu().numpy()[:, 0], A[:, 0], equal_nan=True)
+
+
+def test_checked_build_runs_clean(mc):
+    """SURVEY section 5 (sanitizers): compute-sanitizer is closed on this GPU pool, so the library has a checked build
+    (-DMC_CHECKED, built by __graft_entry__.build()): every index and pointer is tested before the global access that
+    uses it (mc_debug_check).  tests/checked_cases.py drives 40-odd representative launches through it in a process of
+    its own; the product library must say it has no checks (-1)."""
+    import os
+    import subprocess
+    import sys
+    from paper_1802_00147_b200 import build
+    with mc.Integrator() as I:
+        I.integrate(workloads.config0(8).states, 1.0, 10, 3)
+        assert I.debug_check() == -1
+    lib = build.build_checked()
+    env = dict(os.environ, MC_LIBMC_PATH=lib)
+    script = os.path.join(os.path.dirname(os.path.abspath(__file__)), "checked_cases.py")
+    r = subprocess.run([sys.executable, script], env=env, capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-4000:]
+    assert "launches clean" in r.stdout

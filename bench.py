@@ -283,6 +283,7 @@ def run_mc(args):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
 
     peak_tf, peak_clock = binding.fp64_peak(local, 200.0) if rank == 0 else (None, None)
+    probe = binding.fp64_probe(local, 50.0) if rank == 0 else None      # operand-bandwidth rule of the FP64 pipe, measured here
     if w.uniform:
         par = dict(beta=float(w.beta[0]), chi1=float(w.chi1[0]), chi2=float(w.chi2[0]), kq1=float(w.kq1[0]), kq2=float(w.kq2[0]))
     else:
@@ -373,6 +374,7 @@ def run_mc(args):
                                "(MEASURED_PEAKS.json has no FP64 entry)",
                 "peak_measured_dfma": peak_tf, "frac_of_measured_dfma": achieved_tf / peak_tf if peak_tf else None,
                 "dfma_probe_implied_sm_mhz": peak_clock,
+                "fp64_operand_probe": {k: {"cycles_per_warp_instr": v[0], "tflops": v[1]} for k, v in probe.items()} if probe else None,
                 "flop_per_launch": flop_per_launch, "flop_per_orbit_step": flop_per_launch / max(steps_done, 1.0),
                 "flop_model": alg["model"], "flop_model_ops": alg["model_ops"],
                 "flop_source": "mc_flop_model: the kernels' math templates run with a counting scalar (tests/test_flop_model.py)",

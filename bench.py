@@ -56,6 +56,8 @@ def parse_args():
                     help="correction mode override (default: the workload's own, 3 = six-integral projection; profiles/ tables only)")
     ap.add_argument("--sample-interval", type=int, default=0,
                     help="mc_integrate_sampled: record every orbit every K steps (profiles/ tables only; 0 = off)")
+    ap.add_argument("--regroup", action="store_true",
+                    help="mc_params.regroup: integrate the orbits in energy order (index mapping only; profiles/ tables only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -289,7 +291,7 @@ def run_mc(args):
     else:
         par = {k: v for k, v in w.params().items() if k != "terms"}
     rk5 = args.integrator == "rk5"
-    I = binding.Integrator(terms=w.terms, device=local, integrator=int(rk5), **par)
+    I = binding.Integrator(terms=w.terms, device=local, integrator=int(rk5), regroup=int(args.regroup), **par)
     out = torch.empty_like(z_dev)
     stream = torch.cuda.current_stream(dev)
     launches = 0
@@ -394,6 +396,7 @@ def run_mc(args):
                        "orbits_per_gpu": n, "rk4_steps": w.n_steps, "sample_interval": args.sample_interval,
                        "sample_bytes_per_launch": (w.n_steps // args.sample_interval) * 96 * n if args.sample_interval else 0,
                        "orbit_steps_counted": "accepted steps (sum of steps_done); scheduled = orbits x rk4_steps = %d" % int(orbit_steps_rank * world), "l2": "flushed (256 MiB write) between timed iterations",
+                       "regroup": bool(args.regroup),
                        "parallelism": f"orbit-sharded x{world} (grid rows round-robin over ranks), no collective"},
             "clocks": clocks, "wall_s_timed_region": t_wall,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},

@@ -110,11 +110,21 @@ typedef struct mc_params {
                               resources the assumption can fail; a wait longer than this many seconds then ends the
                               launch with a trap (MC_ECUDA on the next call) instead of a hang.  Raise it for
                               profiler replays or very long forced chunks (chunk_steps); must be in (0, 1e9]   */
+  int32_t regroup;         /* scheduling only, never changes a result bit; 0 (default) or 1.  1: mc_integrate first
+                              sorts the orbits by their energy H at t = 0 on the device (one small kernel + a
+                              radix sort, stream-ordered) and lets slot s of the launch integrate the s-th orbit
+                              in that order; inputs and outputs keep the caller's order.  Orbits of equal energy
+                              have equal radial periods to 1PN order, so the 16 orbits of a warp keep passing
+                              periastron together and need their second Gauss-Newton step at the same steps.
+                              Pays for UNSTRUCTURED batches (random initial conditions: +7 %, DESIGN.md section
+                              10); a grid scan in row-major order is already grouped and loses a few per cent.
+                              Ignored with sampled output, by mc_integrate_ex and below 64 orbits             */
+  int32_t reserved_;       /* 0                                                                            */
 } mc_params;
 
 /* Fill *p with defaults: terms = 1PN|2PN|SO|S1S2, device 0, uniform beta = chi = kq = 1,
  * renorm_interval 100, newton_iters 4, newton_tol 1e-10, r_merge 2, r_escape 1e4, stream NULL,
- * chunk_steps 0, integrator RK4, wait_budget_s 600. */
+ * chunk_steps 0, integrator RK4, wait_budget_s 600, regroup 0. */
 int mc_params_default(mc_params* p);
 
 /* Validate params, select the device, allocate the handle.  *out_handle is set only on success. */
@@ -136,7 +146,7 @@ int mc_create(const mc_params* params, mc_handle** out_handle);
  *   out_fli         DEVICE, double[n_orbits]; required iff shadow_eps != 0
  *
  * The call is asynchronous on params.cuda_stream: one kernel launch (preceded by one memset of the
- * work-queue scratch), no host synchronisation, no host<->device copy.  All buffers are owned by the caller.  n_orbits = 0 or n_steps = 0 are valid
+ * work-queue scratch and, with params.regroup, by the key kernel and the sort), no host synchronisation, no host<->device copy.  All buffers are owned by the caller.  n_orbits = 0 or n_steps = 0 are valid
  * (n_steps = 0 copies the normalised state and evaluates the invariants).  Numerical failures of
  * single orbits are not errors: see mc_get_status.
  * Errors: MC_EINVAL (null/negative arguments, n_steps >= 2^31, unknown mode, non-finite step_h), MC_ECUDA. */
@@ -230,7 +240,7 @@ typedef struct mc_launch_info {
   int32_t blocks_per_sm;        /* occupancy API result for that block size       */
   int32_t num_sms;
   int32_t smem_bytes;           /* dynamic shared memory per block                */
-  int32_t variant;              /* bit0 per-orbit params, bit1 QM, bit2 per-orbit kq only, bit3 2.5PN, bits 4-5 mode, bit 8 RK5 */
+  int32_t variant;              /* bit0 per-orbit params, bit1 QM, bit2 per-orbit kq only, bit3 2.5PN, bits 4-5 mode, bit 8 RK5, bit 10 regrouped */
   int64_t trajectories;         /* threads doing work = n_orbits * (1 + shadow)   */
   int32_t chunk_steps;          /* steps per work item                             */
   int32_t n_chunks;             /* work items per 32-trajectory unit              */

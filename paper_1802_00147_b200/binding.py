@@ -39,7 +39,7 @@ class mc_params(ctypes.Structure):
                 ("d_kq1", ctypes.c_void_p), ("d_kq2", ctypes.c_void_p), ("renorm_interval", ctypes.c_int32),
                 ("newton_iters", ctypes.c_int32), ("newton_tol", ctypes.c_double), ("r_merge", ctypes.c_double),
                 ("r_escape", ctypes.c_double), ("cuda_stream", ctypes.c_void_p), ("chunk_steps", ctypes.c_int32), ("integrator", ctypes.c_int32),
-                ("wait_budget_s", ctypes.c_double)]
+                ("wait_budget_s", ctypes.c_double), ("regroup", ctypes.c_int32), ("reserved_", ctypes.c_int32)]
 
 
 class mc_launch_info(ctypes.Structure):
@@ -173,7 +173,7 @@ class Integrator:
 
     def __init__(self, terms=TERMS_DEFAULT, beta=1.0, chi1=1.0, chi2=1.0, kq1=1.0, kq2=1.0, device=0,
                  renorm_interval=100, newton_iters=4, newton_tol=1e-10, r_merge=2.0, r_escape=1e4, stream=None,
-                 chunk_steps=0, integrator=0, wait_budget_s=600.0, per_orbit=None):
+                 chunk_steps=0, integrator=0, wait_budget_s=600.0, per_orbit=None, regroup=0):
         import torch
         self._torch = torch
         self._lib = load_library()
@@ -184,6 +184,7 @@ class Integrator:
         p.chunk_steps = int(chunk_steps)
         p.integrator = int(integrator)
         p.wait_budget_s = float(wait_budget_s)
+        p.regroup = int(regroup)
         self.device = torch.device("cuda", device)
         vals = dict(beta=beta, chi1=chi1, chi2=chi2, kq1=kq1, kq2=kq2)
 

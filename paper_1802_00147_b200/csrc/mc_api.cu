@@ -1,6 +1,7 @@
 // mc_api.cu -- the C ABI of include/mc.h: handle, validation, launches, host-buffer variant,
 // evaluation entry point for the parity tests, FP64 peak probe.
 #include <cuda_runtime.h>
+#include <cub/device/device_radix_sort.cuh>
 
 #include <cmath>
 #include <cstdio>
@@ -56,6 +57,7 @@ struct mc_handle {
   int64_t last_n;            // orbits of the last mc_integrate (status buffers valid for these)
   DeviceBuf status, step, gn, diss;   // int32[n], int64[n], int64[n], double[4][n] (MC_TERM_RR)
   DeviceBuf sched, carry_d, carry_i, carry_g;   // work queue + per-unit flags; carried state between chunks
+  DeviceBuf rg_keys, rg_idx, rg_tmp;            // mc_params.regroup: energy keys (2 x n doubles), slot -> orbit maps (2 x n int32), sort scratch
   DeviceBuf h_in, h_out, h_inv, h_fli;   // scratch of mc_integrate_host
   mc_launch_info info;
 };
@@ -117,6 +119,29 @@ eval_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ mc::Int
 #pragma unroll
     for (int i = 0; i < 16; ++i)
       if (i < rows) out[(int64_t)i * A.n + o] = f[i];
+  }
+}
+
+// ---- mc_params.regroup: energy of every orbit at t = 0 as a sort key ---------------------------------
+// Orbits of equal energy have equal radial periods to 1PN order, so neighbours in energy order keep passing periastron
+// together and a warp's lanes need their second Gauss-Newton step at the same steps.
+template <int PARAMS, bool QM>
+__global__ void __launch_bounds__(mc::kBlock)
+energy_key_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ mc::IntegrateArgs A, double* __restrict__ keys,
+                  int32_t* __restrict__ idx) {
+  extern __shared__ double smem[];
+  const int64_t t = (int64_t)blockIdx.x * mc::kBlock + threadIdx.x;
+  const bool active = t < A.n;
+  const int64_t o = active ? t : A.n - 1;
+  using CP = typename mc::ConstsOf<PARAMS>::type;
+  const CP c = mc::make_consts<PARAMS, CP>(uc, A, o, smem);
+  double z[12];
+#pragma unroll
+  for (int i = 0; i < 12; ++i) z[i] = A.states[(int64_t)i * A.n + o];
+  const double H = mc::hamiltonian<QM>(c, z);
+  if (active) {
+    keys[t] = H;
+    idx[t] = (int32_t)t;
   }
 }
 
@@ -211,6 +236,7 @@ int mc_params_default(mc_params* p) {
   p->chunk_steps = 0;
   p->integrator = MC_INTEG_RK4;
   p->wait_budget_s = 600.0;
+  p->regroup = 0;
   return MC_OK;
 }
 
@@ -223,6 +249,7 @@ int mc_create(const mc_params* params, mc_handle** out_handle) {
   if (params->integrator != MC_INTEG_RK4 && params->integrator != MC_INTEG_RK5) return MC_EINVAL;
   if (!(params->newton_tol >= 0.0) || !(params->r_merge >= 0.0) || !(params->r_escape > params->r_merge)) return MC_EINVAL;
   if (!(params->wait_budget_s > 0.0) || !(params->wait_budget_s <= 1e9)) return MC_EINVAL;
+  if (params->regroup != 0 && params->regroup != 1) return MC_EINVAL;
   if (params->per_orbit < 0 || params->per_orbit > 2) return MC_EINVAL;
   if (params->per_orbit == 1) {
     if (!params->d_beta || !params->d_chi1 || !params->d_chi2 || !params->d_kq1 || !params->d_kq2) return MC_EINVAL;
@@ -368,6 +395,35 @@ static int integrate_impl(mc_handle* h, const double* states, int64_t n_orbits, 
     if ((rc = h->carry_g.reserve(sizeof(unsigned long long) * 2 * tp))) return rc;
     A.carry_d = (double*)h->carry_d.p; A.carry_i = (int32_t*)h->carry_i.p; A.carry_g = (unsigned long long*)h->carry_g.p;
   }
+  A.perm = nullptr;
+  if (h->P.regroup && !user_carry && sample_interval == 0 && n_orbits >= 64 && n_orbits <= 0x7fffffffLL) {
+    // slot -> orbit map: orbits in order of their energy at t = 0 (stable radix sort; device-side, stream-ordered)
+    const size_t n = (size_t)n_orbits;
+    if ((rc = h->rg_keys.reserve(sizeof(double) * 2 * n))) return rc;
+    if ((rc = h->rg_idx.reserve(sizeof(int32_t) * 2 * n))) return rc;
+    double* k_in = (double*)h->rg_keys.p;
+    double* k_out = k_in + n;
+    int32_t* i_in = (int32_t*)h->rg_idx.p;
+    int32_t* i_out = i_in + n;
+    size_t tmp_bytes = 0;
+    MC_CUDA(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, k_in, k_out, i_in, i_out, (int)n_orbits, 0, 64, h->stream));
+    if ((rc = h->rg_tmp.reserve(tmp_bytes))) return rc;
+    const int kgrid = (int)((n_orbits + mc::kBlock - 1) / mc::kBlock);
+    const int kp = h->P.per_orbit == 1 ? 1 : ((h->P.per_orbit == 2 && qm) ? 2 : 0);
+    const size_t ksmem = kp == 1 ? sizeof(double) * MC_NCONST * mc::kBlock : 0;
+    if (ksmem > 48 * 1024) {
+      MC_CUDA(cudaFuncSetAttribute(energy_key_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ksmem));
+      MC_CUDA(cudaFuncSetAttribute(energy_key_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ksmem));
+    }
+    if (kp == 1 && qm) energy_key_kernel<1, true><<<kgrid, mc::kBlock, ksmem, h->stream>>>(h->uc, A, k_in, i_in);
+    else if (kp == 1) energy_key_kernel<1, false><<<kgrid, mc::kBlock, ksmem, h->stream>>>(h->uc, A, k_in, i_in);
+    else if (kp == 2) energy_key_kernel<2, true><<<kgrid, mc::kBlock, 0, h->stream>>>(h->uc, A, k_in, i_in);
+    else if (qm) energy_key_kernel<0, true><<<kgrid, mc::kBlock, 0, h->stream>>>(h->uc, A, k_in, i_in);
+    else energy_key_kernel<0, false><<<kgrid, mc::kBlock, 0, h->stream>>>(h->uc, A, k_in, i_in);
+    MC_CUDA(cudaGetLastError());
+    MC_CUDA(cub::DeviceRadixSort::SortPairs(h->rg_tmp.p, tmp_bytes, k_in, k_out, i_in, i_out, (int)n_orbits, 0, 64, h->stream));
+    A.perm = i_out;
+  }
   MC_CUDA(cudaMemsetAsync(h->sched.p, 0, 32 + sizeof(int32_t) * (size_t)A.n_units, h->stream));
   MC_CUDA(fn(h->uc, A, h->num_sms, true, h->stream, &ki));
   h->info.grid = ki.grid;
@@ -380,7 +436,7 @@ static int integrate_impl(mc_handle* h, const double* states, int64_t n_orbits, 
   h->info.num_sms = h->num_sms;
   h->info.smem_bytes = (int32_t)ki.smem;
   const int kparams = (h->P.per_orbit == 2 && !qm) ? 0 : h->P.per_orbit;   // kappa is unused without the QM term
-  h->info.variant = (kparams == 1 ? 1 : 0) | (qm ? 2 : 0) | (kparams == 2 ? 4 : 0) | (rr ? 8 : 0) | (correction_mode << 4) | (h->P.integrator << 8);
+  h->info.variant = (kparams == 1 ? 1 : 0) | (qm ? 2 : 0) | (kparams == 2 ? 4 : 0) | (rr ? 8 : 0) | (correction_mode << 4) | (h->P.integrator << 8) | (A.perm ? 1024 : 0);
   h->info.trajectories = traj;
   return MC_OK;
 }
@@ -578,6 +634,7 @@ int mc_destroy(mc_handle* h) {
   cudaSetDevice(h->P.device);
   h->status.release(); h->step.release(); h->gn.release(); h->diss.release();
   h->sched.release(); h->carry_d.release(); h->carry_i.release(); h->carry_g.release();
+  h->rg_keys.release(); h->rg_idx.release(); h->rg_tmp.release();
   h->h_in.release(); h->h_out.release(); h->h_inv.release(); h->h_fli.release();
   delete h;
   return MC_OK;

@@ -27,6 +27,7 @@ struct IntegrateArgs {
   int64_t* out_step;         // [n]
   int64_t* out_gn;           // [n] Gauss-Newton steps of mode 3 over accepted steps, orbit + shadow
   const double* beta; const double* chi1; const double* chi2; const double* kq1; const double* kq2;  // per-orbit mode
+  const int32_t* perm;       // [n] or null: the orbit that slot s of the launch integrates (mc_params.regroup; scheduling only)
   int64_t n;                 // orbits
   int64_t n_steps;
   double h;
@@ -135,7 +136,9 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
     const int64_t orbit_raw = shadow ? (t >> 1) : t;
     const bool role_shadow = shadow && (t & 1);
     const bool active = orbit_raw < A.n;
-    const int64_t orbit = active ? orbit_raw : (A.n - 1);   // idle lanes shadow-compute a valid orbit, never store
+    const int64_t slot = active ? orbit_raw : (A.n - 1);    // idle lanes shadow-compute a valid orbit, never store
+    MC_CHK(slot >= 0 && slot < A.n);
+    const int64_t orbit = A.perm ? (int64_t)A.perm[slot] : slot;   // which orbit this slot holds: an index mapping only
     MC_CHK(unit >= 0 && unit < A.n_units && chunk >= 0 && chunk < A.n_chunks);
     MC_CHK(t >= 0 && t < tp && orbit >= 0 && orbit < A.n);
     MC_CHK(PARAMS == PARAMS_UNIFORM || (A.kq1 != nullptr && A.kq2 != nullptr));

@@ -51,6 +51,12 @@ def main():
     with binding.Integrator(chunk_steps=100) as I:
         I.integrate(z, 1.0, 1500, 3, shadow_eps=1e-8, sample_interval=100)
         clean(I, "dropped cells")
+    w4 = workloads.config4(12)
+    for n in (64, 1237, 4096):
+        with binding.Integrator(regroup=1, chunk_steps=70) as I:
+            I.integrate(w4.states[:, :n], 1.0, 200, 3, shadow_eps=1e-8)
+            assert I.launch_info()["variant"] & 1024
+            clean(I, f"regroup n={n}")
     wl = workloads.config2(n_r=120, n_theta=314, n_steps=600)                    # 37 680 orbits: more units than resident warps
     with binding.Integrator() as I:
         I.integrate(wl.states, 1.0, 600, 3, shadow_eps=1e-8)

@@ -1007,3 +1007,49 @@ def test_checked_build_runs_clean(mc):
     r = subprocess.run([sys.executable, script], env=env, capture_output=True, text=True, timeout=900)
     assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-4000:]
     assert "launches clean" in r.stdout
+
+
+@pytest.mark.parametrize("case", ["random-shadow", "random-no-shadow-in-place", "per-orbit", "kappa-qm-dropped", "rr", "nan-input"])
+def test_regroup_never_changes_a_bit(mc, case):
+    """mc_params.regroup: slot s of the launch integrates the s-th orbit in energy order.  An
+    index mapping only: every output, in the caller's order, equals the unmapped run bit for bit -- ragged sizes, in
+    place, per-orbit parameters (the mapping carries them along), dropped cells, 2.5PN, a NaN among the inputs."""
+    kw, mode, eps, terms, steps = {}, 3, 1e-8, 15, 700
+    if case == "random-shadow":
+        z = workloads.config4(12).states[:, :1237]
+    elif case == "random-no-shadow-in-place":
+        z, eps = workloads.config4(12).states[:, :333], 0.0
+    elif case == "per-orbit":
+        w = workloads.config1().subset(np.arange(301))
+        z, kw = w.states, {k: v for k, v in w.params().items() if k != "terms"}
+    elif case == "kappa-qm-dropped":
+        w = workloads.config3(n_r=10, n_theta=23, qm=True)
+        z, terms, kw = w.states, w.terms, {k: v for k, v in w.params().items() if k != "terms"}
+        steps = 3000
+    elif case == "rr":
+        z, terms = workloads.config4(12).states[:, :200] * np.array([3.0] * 3 + [3 ** -0.5] * 3 + [1.0] * 6)[:, None], 15 | RR
+    else:
+        z = workloads.config4(12).states[:, :130].copy()
+        z[2, 77] = np.nan
+    n = z.shape[1]
+    outs = {}
+    for rg in (0, 1):
+        with mc.Integrator(terms=terms, regroup=rg, chunk_steps=(90 if rg else 0), **kw) as I:
+            if case == "random-no-shadow-in-place":
+                zt = torch.as_tensor(z, device="cuda").clone()
+                g = I.integrate(zt, 1.0, steps, mode, shadow_eps=eps, out_states=zt)
+            else:
+                g = I.integrate(z, 1.0, steps, mode, shadow_eps=eps)
+            info = I.launch_info()
+            extra = [I.work(n).cpu().numpy()] + ([I.dissipation(n).cpu().numpy()] if terms & RR else [])
+        assert bool(info["variant"] & 1024) == bool(rg)
+        outs[rg] = [t.cpu().numpy() for t in (g.states, g.invariants, g.status, g.steps_done)] + extra + ([g.fli.cpu().numpy()] if eps else [])
+    if case == "kappa-qm-dropped":
+        assert (outs[0][2] != 0).sum() >= 10
+    if case == "nan-input":
+        assert outs[0][2][77] == 3 and (np.delete(outs[0][2], 77) == 0).all()
+    for a, b in zip(outs[0], outs[1]):
+        assert np.array_equal(a, b, equal_nan=True), case
+    with mc.Integrator(regroup=1) as I:                       # below 64 orbits the mapping is not worth a sort: ignored
+        I.integrate(z[:, :40], 1.0, 10, 3, shadow_eps=1e-8)
+        assert not (I.launch_info()["variant"] & 1024)

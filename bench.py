@@ -380,6 +380,10 @@ def run_mc(args):
                 "flop_per_launch": flop_per_launch, "flop_per_orbit_step": flop_per_launch / max(steps_done, 1.0),
                 "flop_model": alg["model"], "flop_model_ops": alg["model_ops"],
                 "flop_source": "mc_flop_model: the kernels' math templates run with a counting scalar (tests/test_flop_model.py)",
+                # continuity with BENCH_r01 (config 2, RK4, mode 3, QM off only): round 1's frozen hand count, 2270 per orbit-step +
+                # 390 per Gauss-Newton step, counted the rsqrt / reciprocal refinements as algorithmic work
+                "frac_with_round1_hand_count": ((2270.0 * steps_done + 390.0 * gn_steps) / per_launch_s / 1e12 / nominal_tf
+                                                if (traj == 2 and w.correction_mode == 3 and not rk5 and not (w.terms & 48)) else None),
                 "gn_steps_per_trajectory_step": gn_steps / max(traj * steps_done, 1.0),
                 "executed": executed,
                 "accepted_orbit_steps_per_launch": steps_done, "kernel": "mc::integrate_kernel<%s,QM %s,mode %d,%s%s>" % (

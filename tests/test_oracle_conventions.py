@@ -131,3 +131,39 @@ def test_conservative_runs_are_bit_identical_to_the_stored_oracle_outputs():
     got = list(mod.lines())
     assert len(want) == len(got) == 6 * len(mod.CASES)
     assert got == want
+
+
+def test_dual_scaling_skip_policy_and_root_selection():
+    """DESIGN.md R7 (mode 2, the paper's eqs 11-13): (i) the scaling is applied only while |v - 1| <= 1e-3, else the step is
+    skipped and (r, p) stay untouched; (ii) of the two roots of the |J| quadratic the one continuous with gamma = 1 is
+    taken, also when the spins are anti-aligned with and larger than L (sigma = -1).  Both found unpinned by a mutation run
+    over oracle/pn_oracle.hpp (round 2).  Constructed cases: the exact root is known because r -> r / v, p -> v p leaves
+    L, hence |J|, unchanged, so E0 := H at the scaled state makes v the root."""
+    par = dict(beta=1.0, chi1=0.9, chi2=0.8, terms=15)
+    z = workloads.paper_orbit(4).states
+    J0 = oracle.total_J(z, **par)
+    for v, applied in ((1 + 5e-4, True), (1 - 8e-4, True), (1 + 1.5e-3, False), (1 - 1.5e-3, False)):
+        zs = z.copy()
+        zs[0:3] /= v
+        zs[3:6] *= v
+        E0 = oracle.hamiltonian(zs, **par)
+        got, ok = oracle.correct(z, E0, J0, 2, newton_iters=8, **par)
+        assert bool(ok[0]) == applied, v
+        want = zs if applied else z
+        assert np.abs(got[0:6] - want[0:6]).max() < 1e-13 * np.abs(z[0:3]).max(), v
+    # (ii) L = 0.15 z_hat, S1 = -0.9 z_hat, S2 = -0.8 z_hat: L.L + L.S < 0.  On the manifold the correction is the identity;
+    # the other root of the quadratic (gamma = -1 - 2 L.S / L.L = 21.7) would throw the orbit away or skip.
+    y = np.zeros((12, 1))
+    y[0], y[4], y[8], y[11] = 3.0, 0.05, -1.0, -1.0
+    E0, J0 = oracle.hamiltonian(y, **par), oracle.total_J(y, **par)
+    assert (J0[2] < 0).all()
+    got, ok = oracle.correct(y, E0, J0, 2, newton_iters=4, **par)
+    assert ok[0] == 1 and np.abs(got - y).max() < 1e-14
+    yp = y.copy()
+    yp[0:3] *= 1 + 2e-4
+    yp[3:6] *= 1 - 1e-4                       # off the manifold: E and |J| are restored with gamma close to 1
+    got, ok = oracle.correct(yp, E0, J0, 2, newton_iters=6, **par)
+    I1 = oracle.integrals(got, **par)
+    assert ok[0] == 1 and abs(I1[0, 0] / E0[0] - 1) < 1e-14
+    assert abs(np.linalg.norm(I1[1:4, 0]) / np.linalg.norm(J0[:, 0]) - 1) < 1e-14
+    assert abs(got[4, 0] / yp[4, 0] - 1) < 1e-2                               # gamma v ~ 1, not ~ 20

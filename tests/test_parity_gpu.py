@@ -1053,3 +1053,34 @@ def test_regroup_never_changes_a_bit(mc, case):
     with mc.Integrator(regroup=1) as I:                       # below 64 orbits the mapping is not worth a sort: ignored
         I.integrate(z[:, :40], 1.0, 10, 3, shadow_eps=1e-8)
         assert not (I.launch_info()["variant"] & 1024)
+
+
+def test_dual_scaling_skip_policy_and_root_selection_match_the_oracle(mc):
+    """DESIGN.md R7 on the kernel's side: the constructed cases of tests/test_oracle_conventions.py
+    (test_dual_scaling_skip_policy_and_root_selection) through mc_eval -- scaling applied for |v - 1| <= 1e-3, skipped
+    with (r, p) untouched beyond, and the root continuous with gamma = 1 when L.L + L.S < 0."""
+    par = dict(beta=1.0, chi1=0.9, chi2=0.8)
+    z = workloads.paper_orbit(4).states
+    J0 = oracle.total_J(z, terms=15, **par)
+    states, refs = [], []
+    for v in (1 + 5e-4, 1 - 8e-4, 1 + 1.5e-3, 1 - 1.5e-3):
+        zs = z.copy()
+        zs[0:3] /= v
+        zs[3:6] *= v
+        states.append(z)
+        refs.append(np.concatenate([oracle.hamiltonian(zs, terms=15, **par)[None], J0], axis=0))
+    y = np.zeros((12, 1))
+    y[0], y[4], y[8], y[11] = 3.0, 0.05, -1.0, -1.0
+    Ry = np.concatenate([oracle.hamiltonian(y, terms=15, **par)[None], oracle.total_J(y, terms=15, **par)], axis=0)
+    yp = y.copy()
+    yp[0:3] *= 1 + 2e-4
+    yp[3:6] *= 1 - 1e-4
+    states += [y, yp]
+    refs += [Ry, Ry]
+    Z, R = np.concatenate(states, axis=1), np.concatenate(refs, axis=1)
+    want, ok = oracle.correct(Z, R[0], R[1:4], 2, newton_iters=6, terms=15, **par)
+    assert list(ok) == [1, 1, 0, 0, 1, 1]
+    with mc.Integrator(newton_iters=6, **par) as I:
+        got = I.eval("correct", Z, mode=2, refs=R).cpu().numpy()
+    assert rel_state_err(got, want) < 1e-12
+    assert np.array_equal(got[0:6, 2:4], Z[0:6, 2:4])                    # skipped: (r, p) untouched, bit for bit

@@ -67,7 +67,10 @@ __device__ __forceinline__ double rcp_nz(double x) {
   return fma(y, e, y);
 }
 __device__ __forceinline__ double sqrt_pos(double x) { return sqrt(x); }
-__device__ __forceinline__ double div_(double a, double b) { return a / b; }
+// a / b for mode 2's quadratic root and Newton updates: a times the refined reciprocal (<= 1.5 ulp; no IEEE division
+// sequence with its slow path in the step loop).  b = 0 or non-finite gives a non-finite result, which the caller's
+// skip test catches just as it would after a true division.
+__device__ __forceinline__ double div_(double a, double b) { return a * rcp_nz(b); }
 __device__ __forceinline__ bool is_finite(double v) { return (((unsigned)__double2hiint(v)) & 0x7ff00000u) != 0x7ff00000u; }
 
 __device__ __forceinline__ bool finite12(const double* z) {

@@ -21,7 +21,14 @@
 // chi_i m_i^2 in units of mu*M (reading R2).
 //
 // Pins for every function in this file: tests/test_oracle_*.py (see the table
-// in DESIGN.md section "Oracle pins").
+// in DESIGN.md section "Oracle pins"; a 480-mutant run over this file is
+// recorded there).
+// Parity unpinned (readings PAPER.md cannot fix, shared by both sides, listed in
+// DESIGN.md section 6.3): the gauge (A, B) of the 2.5PN force in rr_force (R21:
+// the paper does not print the expression; every gauge-invariant consequence is
+// pinned), the unweighted 12-component norm of the FLI distance (R12), the
+// identity metric of the mode-3 projection (R14), and the regular / chaotic
+// labels the paper prints for its own orbits (R19 note).
 #pragma once
 #include <cmath>
 #include <cstdint>

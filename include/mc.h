@@ -43,7 +43,7 @@ enum mc_terms {
                          carries the work W = int (dr/dt).a dt and the torque integral G = int r x a dt of the
                          force, and the correction (modes 2, 3) targets E0 + W and J0 + G, the "integral invariant
                          relation" of PAPER.md:221; see mc_get_dissipation.  Default off.  One combination is not
-                         built: per_orbit = 1 together with MC_INTEG_RK5 (mc_integrate returns MC_EINVAL; the 37
+                         built: per_orbit = 1 together with MC_INTEG_RK5 (mc_integrate returns MC_EINVAL; the 45
                          per-orbit constants, six stages and 16 components exceed the 255-register budget and the
                          library ships no kernel that spills)                                               */
 };

@@ -9,7 +9,7 @@ namespace mc {
 
 // Resident 128-thread blocks per SM the register allocator must allow.  With constant-bank parameters (uniform, or
 // uniform + per-orbit kappa in four registers) the RK4 kernels fit 3 blocks (<= 168 registers) without spills, with
-// or without the quadrupole-monopole term.  Fully per-orbit parameters (37 constants in shared memory) and the
+// or without the quadrupole-monopole term.  Fully per-orbit parameters (45 constants in shared memory) and the
 // six-stage RK5 need <= 255 registers (2 blocks).  ptxas -v: 0 spill bytes for every instantiation (build() raises
 // otherwise).
 #ifndef MC_MINB_UNIFORM
@@ -51,7 +51,7 @@ static cudaError_t launch(const McConsts& uc, const IntegrateArgs& A, int num_sm
 template <int MODE, int INTEG, bool RR>
 static LaunchFn pick3(int params, bool qm) {
   if (params == PARAMS_PER_ORBIT) {
-    // 37 per-orbit constants + six RK5 stages + the 16-component trajectory do not fit 255 registers: that one
+    // 45 per-orbit constants + six RK5 stages + the 16-component trajectory do not fit 255 registers: that one
     // combination is not built (mc_integrate returns MC_EINVAL; include/mc.h, MC_TERM_RR)
     if constexpr (INTEG == 1 && RR) return nullptr;
     else return qm ? launch<PARAMS_PER_ORBIT, true, MODE, INTEG, RR> : launch<PARAMS_PER_ORBIT, false, MODE, INTEG, RR>;

@@ -99,11 +99,11 @@ eval_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ mc::Int
     rows = 6;
   } else if (what == 3) {
     if (rr) {
-      if (A.integrator == 1) mc::rk5_step<QM, true>(c, z, A.h, f);
-      else mc::rk4_step<QM, true>(c, z, A.h, f);
+      if (A.integrator == 1) mc::rk5_step<QM, true>(c, z, A.hw, f);
+      else mc::rk4_step<QM, true>(c, z, A.hw, f);
       rows = 16;
-    } else if (A.integrator == 1) mc::rk5_step<QM, false>(c, z, A.h, f);
-    else mc::rk4_step<QM, false>(c, z, A.h, f);
+    } else if (A.integrator == 1) mc::rk5_step<QM, false>(c, z, A.hw, f);
+    else mc::rk4_step<QM, false>(c, z, A.hw, f);
   } else {
     mc::Refs R;
     R.E0 = refs[o];
@@ -340,7 +340,7 @@ static int integrate_impl(mc_handle* h, const double* states, int64_t n_orbits, 
   A.states = states; A.out_states = out_states; A.out_inv = out_invariants; A.out_fli = shadow ? out_fli : nullptr;
   A.out_status = (int32_t*)h->status.p; A.out_step = (int64_t*)h->step.p; A.out_gn = (int64_t*)h->gn.p;
   A.out_diss = rr ? (double*)h->diss.p : nullptr;
-  A.n = n_orbits; A.n_steps = n_steps; A.h = step_h; A.shadow_eps = shadow_eps;
+  A.n = n_orbits; A.n_steps = n_steps; A.h = step_h; A.hw = mc::step_weights(step_h); A.shadow_eps = shadow_eps;
   A.samples = sample_interval > 0 ? out_samples : nullptr;
   A.sample_interval = sample_interval > 0 ? (int32_t)sample_interval : 1;
 
@@ -531,7 +531,7 @@ int mc_eval(mc_handle* h, int32_t what, const double* states, int64_t n, double 
   MC_CUDA(cudaSetDevice(h->P.device));
   mc::IntegrateArgs A;
   fill_args(h, A);
-  A.states = states; A.n = n; A.h = step_h;
+  A.states = states; A.n = n; A.h = step_h; A.hw = mc::step_weights(step_h);
   const bool qm = (h->P.terms & MC_TERM_QM) != 0, po = h->P.per_orbit == 1, ka = h->P.per_orbit == 2 && qm;
   const int grid = (int)((n + mc::kBlock - 1) / mc::kBlock);
   const size_t smem = po ? sizeof(double) * MC_NCONST * mc::kBlock : 0;

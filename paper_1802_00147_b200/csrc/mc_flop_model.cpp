@@ -43,7 +43,7 @@ void model(const HostConsts& c, int mode, int newton_iters, mc_flop_model_t* out
   Cnt z[16], f[16];
   sample_state(z);
   out->rhs = count([&] { mc::pn_rhs<QM, RR>(c, z, f); });
-  out->base_step = count([&] { mc::base_step<INTEG, QM, RR>(c, z, 1.0, f); });
+  out->base_step = count([&] { mc::base_step<INTEG, QM, RR>(c, z, mc::step_weights(1.0), f); });
   mc::RefsT<Cnt> R;
   mc::references<QM>(c, z, R);
   out->references = count([&] { mc::references<QM>(c, z, R); });

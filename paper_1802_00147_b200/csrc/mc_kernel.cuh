@@ -31,6 +31,7 @@ struct IntegrateArgs {
   int64_t n;                 // orbits
   int64_t n_steps;
   double h;
+  StepWeights hw;            // h times the tableau coefficients (step_weights(h)): constant-bank operands of the stage sums
   double shadow_eps;         // 0: no shadow
   double r_merge2, r_escape2;
   double newton_tol;
@@ -226,7 +227,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
       }
       ++warp_steps;
       double z[NS];
-      base_step<INTEG, QM, RR>(c, y, A.h, z);
+      base_step<INTEG, QM, RR>(c, y, A.hw, z);
       int gn, gnw;
       bool ok;
       if constexpr (RR) {   // the manifold has moved by the work and torque of the step (integral invariant relation)

@@ -235,32 +235,51 @@ MC_DEV T hamiltonian(const C& c, const T* z) {
   return H;
 }
 
+// Step weights: h times the coefficients of the two tableaus, formed once on the host (mc_api.cu) and carried in the
+// kernel parameter.  The stage inputs y + (h c) k and the running sum of b_i k_i are 84 FMAs per RK4 step; with the
+// weight in the constant bank each reads two registers (2 cycles on the FP64 pipe), with the weight in a register
+// three (3 cycles, operand bandwidth).  The products are the ones the step routines used to
+// form themselves in double precision, so results do not change by a bit.
+enum McStepWeightIndex {
+  HW_H = 0, HW_H2, HW_H3, HW_H6,                                                        // RK4: h, h/2, h/3, h/6
+  HW_H790, HW_H3290, HW_H1290, HW_H4, HW_H8, HW_HM2, HW_H37, HW_H27, HW_H127, HW_H316, HW_H916, HW_H87   // RK5
+};
+struct StepWeights { double v[16]; };
+MC_HD StepWeights step_weights(double h) {
+  StepWeights w;
+  w.v[HW_H] = h; w.v[HW_H2] = 0.5 * h; w.v[HW_H3] = h * (1.0 / 3.0); w.v[HW_H6] = h * (1.0 / 6.0);
+  w.v[HW_H790] = h * (7.0 / 90.0); w.v[HW_H3290] = h * (32.0 / 90.0); w.v[HW_H1290] = h * (12.0 / 90.0);
+  w.v[HW_H4] = 0.25 * h; w.v[HW_H8] = 0.125 * h; w.v[HW_HM2] = -0.5 * h;
+  w.v[HW_H37] = h * (-3.0 / 7.0); w.v[HW_H27] = h * (2.0 / 7.0); w.v[HW_H127] = h * (12.0 / 7.0);
+  w.v[HW_H316] = h * (3.0 / 16.0); w.v[HW_H916] = h * (9.0 / 16.0); w.v[HW_H87] = h * (8.0 / 7.0);
+  return w;
+}
+
 // Classical RK4 (R9), low-storage bookkeeping: y (kept), acc, stage input yt.
 // RR: components 12-15 (W, G) never enter the right-hand side, so they need no stage inputs: only their weighted
 // sum of stage derivatives is accumulated.
 template <bool QM, bool RR, class C, class T>
-MC_DEV void rk4_step(const C& c, const T* y, double h, T* out) {
+MC_DEV void rk4_step(const C& c, const T* y, const StepWeights& w, T* out) {
   constexpr int NS = RR ? 16 : 12;
-  const double h2 = 0.5 * h, h3 = h * (1.0 / 3.0), h6 = h * (1.0 / 6.0);
   T k[NS], yt[12];
   pn_rhs<QM, RR>(c, y, k);
 #pragma unroll
-  for (int i = 0; i < NS; ++i) out[i] = fma(h6, k[i], y[i]);
+  for (int i = 0; i < NS; ++i) out[i] = fma(w.v[HW_H6], k[i], y[i]);
 #pragma unroll
-  for (int i = 0; i < 12; ++i) yt[i] = fma(h2, k[i], y[i]);
+  for (int i = 0; i < 12; ++i) yt[i] = fma(w.v[HW_H2], k[i], y[i]);
   pn_rhs<QM, RR>(c, yt, k);
 #pragma unroll
-  for (int i = 0; i < NS; ++i) out[i] = fma(h3, k[i], out[i]);
+  for (int i = 0; i < NS; ++i) out[i] = fma(w.v[HW_H3], k[i], out[i]);
 #pragma unroll
-  for (int i = 0; i < 12; ++i) yt[i] = fma(h2, k[i], y[i]);
+  for (int i = 0; i < 12; ++i) yt[i] = fma(w.v[HW_H2], k[i], y[i]);
   pn_rhs<QM, RR>(c, yt, k);
 #pragma unroll
-  for (int i = 0; i < NS; ++i) out[i] = fma(h3, k[i], out[i]);
+  for (int i = 0; i < NS; ++i) out[i] = fma(w.v[HW_H3], k[i], out[i]);
 #pragma unroll
-  for (int i = 0; i < 12; ++i) yt[i] = fma(h, k[i], y[i]);
+  for (int i = 0; i < 12; ++i) yt[i] = fma(w.v[HW_H], k[i], y[i]);
   pn_rhs<QM, RR>(c, yt, k);
 #pragma unroll
-  for (int i = 0; i < NS; ++i) out[i] = fma(h6, k[i], out[i]);
+  for (int i = 0; i < NS; ++i) out[i] = fma(w.v[HW_H6], k[i], out[i]);
 }
 
 // Butcher's six-stage fifth-order method (the paper's "RK5", R9):
@@ -270,59 +289,53 @@ MC_DEV void rk4_step(const C& c, const T* y, double h, T* out) {
 // the stages arrive, so at most five 12-vectors are live besides the derivative being computed.  RR: components
 // 12-15 only accumulate the final sum (see rk4_step).
 template <bool QM, bool RR, class C, class T>
-MC_DEV void rk5_step(const C& c, const T* y, double h, T* out) {
+MC_DEV void rk5_step(const C& c, const T* y, const StepWeights& w, T* out) {
   constexpr int NS = RR ? 16 : 12;
   T k[NS], k1[12], yt[12], A4[12], S6[12];
-  const double h790 = h * (7.0 / 90.0), h3290 = h * (32.0 / 90.0), h1290 = h * (12.0 / 90.0);
   pn_rhs<QM, RR>(c, y, k);
-  const double h4 = 0.25 * h, h8 = 0.125 * h;
 #pragma unroll
-  for (int i = 0; i < 12; ++i) { k1[i] = k[i]; yt[i] = fma(h4, k[i], y[i]); }
+  for (int i = 0; i < 12; ++i) { k1[i] = k[i]; yt[i] = fma(w.v[HW_H4], k[i], y[i]); }
 #pragma unroll
-  for (int i = 12; i < NS; ++i) out[i] = fma(h790, k[i], y[i]);
+  for (int i = 12; i < NS; ++i) out[i] = fma(w.v[HW_H790], k[i], y[i]);
   pn_rhs<QM, RR>(c, yt, k);                                                    // k2 (b2 = 0)
-  const double hm2 = -0.5 * h, h37 = h * (-3.0 / 7.0), h27 = h * (2.0 / 7.0);
 #pragma unroll
   for (int i = 0; i < 12; ++i) {
-    yt[i] = fma(h8, k[i], fma(h8, k1[i], y[i]));
-    A4[i] = fma(hm2, k[i], y[i]);
-    S6[i] = fma(h27, k[i], fma(h37, k1[i], y[i]));
+    yt[i] = fma(w.v[HW_H8], k[i], fma(w.v[HW_H8], k1[i], y[i]));
+    A4[i] = fma(w.v[HW_HM2], k[i], y[i]);
+    S6[i] = fma(w.v[HW_H27], k[i], fma(w.v[HW_H37], k1[i], y[i]));
   }
   pn_rhs<QM, RR>(c, yt, k);                                                    // k3
-  const double h127 = h * (12.0 / 7.0);
 #pragma unroll
   for (int i = 0; i < 12; ++i) {
-    yt[i] = fma(h, k[i], A4[i]);
-    S6[i] = fma(h127, k[i], S6[i]);
-    out[i] = fma(h3290, k[i], fma(h790, k1[i], y[i]));
+    yt[i] = fma(w.v[HW_H], k[i], A4[i]);
+    S6[i] = fma(w.v[HW_H127], k[i], S6[i]);
+    out[i] = fma(w.v[HW_H3290], k[i], fma(w.v[HW_H790], k1[i], y[i]));
   }
 #pragma unroll
-  for (int i = 12; i < NS; ++i) out[i] = fma(h3290, k[i], out[i]);
+  for (int i = 12; i < NS; ++i) out[i] = fma(w.v[HW_H3290], k[i], out[i]);
   pn_rhs<QM, RR>(c, yt, k);                                                    // k4
-  const double h316 = h * (3.0 / 16.0), h916 = h * (9.0 / 16.0);
 #pragma unroll
   for (int i = 0; i < 12; ++i) {
-    yt[i] = fma(h916, k[i], fma(h316, k1[i], y[i]));
-    S6[i] = fma(-h127, k[i], S6[i]);
+    yt[i] = fma(w.v[HW_H916], k[i], fma(w.v[HW_H316], k1[i], y[i]));
+    S6[i] = fma(-w.v[HW_H127], k[i], S6[i]);
   }
 #pragma unroll
-  for (int i = 0; i < NS; ++i) out[i] = fma(h1290, k[i], out[i]);
+  for (int i = 0; i < NS; ++i) out[i] = fma(w.v[HW_H1290], k[i], out[i]);
   pn_rhs<QM, RR>(c, yt, k);                                                    // k5
-  const double h87 = h * (8.0 / 7.0);
 #pragma unroll
-  for (int i = 0; i < 12; ++i) yt[i] = fma(h87, k[i], S6[i]);
+  for (int i = 0; i < 12; ++i) yt[i] = fma(w.v[HW_H87], k[i], S6[i]);
 #pragma unroll
-  for (int i = 0; i < NS; ++i) out[i] = fma(h3290, k[i], out[i]);
+  for (int i = 0; i < NS; ++i) out[i] = fma(w.v[HW_H3290], k[i], out[i]);
   pn_rhs<QM, RR>(c, yt, k);                                                    // k6
 #pragma unroll
-  for (int i = 0; i < NS; ++i) out[i] = fma(h790, k[i], out[i]);
+  for (int i = 0; i < NS; ++i) out[i] = fma(w.v[HW_H790], k[i], out[i]);
 }
 
 // INTEG: 0 classical RK4, 1 Butcher RK5
 template <int INTEG, bool QM, bool RR, class C, class T>
-MC_DEV void base_step(const C& c, const T* y, double h, T* out) {
-  if (INTEG == 1) rk5_step<QM, RR>(c, y, h, out);
-  else rk4_step<QM, RR>(c, y, h, out);
+MC_DEV void base_step(const C& c, const T* y, const StepWeights& w, T* out) {
+  if (INTEG == 1) rk5_step<QM, RR>(c, y, w, out);
+  else rk4_step<QM, RR>(c, y, w, out);
 }
 
 // eq (10): sigma <- sigma / |sigma|

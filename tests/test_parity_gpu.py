@@ -15,6 +15,10 @@ pytestmark = pytest.mark.gpu
 STATE_RTOL = 1e-10      # north_star
 DRIFT_TOL = 1e-12       # north_star
 FLI_THRESHOLD = 5.8
+# FLI value after 1e3-2e3 steps (north_star states no tolerance for the value, only for the class):
+# about three times the deviation of the oracle's own double instance from its long-double instance on the same inputs
+# (0.8e-3 .. 1.3e-3, pinned on CPU by test_fli_rounding_envelope_sets_the_parity_bound)
+FLI_VALUE_TOL = 3e-3
 
 
 @pytest.fixture(scope="module")
@@ -137,7 +141,7 @@ def test_config1_shadow_fli_parity_per_orbit_params(mc, mode):
         work = I.work(w.n_orbits).cpu().numpy()
     o = oracle.integrate(w.states, w.h, 2000, mode, shadow_eps=w.shadow_eps, **w.params())
     assert rel_state_err(g.states.cpu().numpy(), o.states) <= 4 * STATE_RTOL   # 2e3 steps
-    assert np.abs(g.fli.cpu().numpy() - o.fli).max() < 1e-3
+    assert np.abs(g.fli.cpu().numpy() - o.fli).max() < FLI_VALUE_TOL
     assert np.array_equal(g.status.cpu().numpy(), o.status)
     assert np.array_equal(g.steps_done.cpu().numpy(), o.steps_done)
     if mode == 3:
@@ -192,7 +196,7 @@ def test_config3_quadrupole_on_off_parity(mc):
         ok = o.status == 0
         assert np.array_equal(g.status.cpu().numpy(), o.status)
         assert rel_state_err(g.states.cpu().numpy()[:, ok], o.states[:, ok]) <= STATE_RTOL
-        assert np.abs(g.fli.cpu().numpy()[ok] - o.fli[ok]).max() < 1e-3
+        assert np.abs(g.fli.cpu().numpy()[ok] - o.fli[ok]).max() < FLI_VALUE_TOL
         out[qm] = g.states.cpu().numpy()
     assert np.abs(out[True] - out[False]).max() > 1e-3          # the term really changes the dynamics
 
@@ -224,7 +228,7 @@ def test_per_orbit_kappa_variant_matches_oracle_and_the_full_per_orbit_kernel(mc
         assert info["blocks_per_sm"] == (3 if force is None else 2)
         assert np.array_equal(g.status.cpu().numpy(), o.status)
         assert rel_state_err(g.states.cpu().numpy()[:, ok], o.states[:, ok]) <= STATE_RTOL
-        assert np.abs(g.fli.cpu().numpy()[ok] - o.fli[ok]).max() < 1e-3
+        assert np.abs(g.fli.cpu().numpy()[ok] - o.fli[ok]).max() < FLI_VALUE_TOL
         assert drift(g.states.cpu().numpy()[:, ok], o.invariants[0:6][:, ok], **w.subset(np.where(ok)[0]).params()) <= DRIFT_TOL
         got[force] = g.states.cpu().numpy()
     assert rel_state_err(got[None][:, ok], got[1][:, ok]) <= STATE_RTOL
@@ -292,7 +296,7 @@ def test_non_unit_input_spins(mc, mode):
         assert np.array_equal(gs, o.status)
     err = rel_state_err(gz[:, clean], o.states[:, clean])
     assert err <= (5e-10 if mode == 2 else STATE_RTOL), err
-    assert np.abs(g.fli.cpu().numpy()[clean] - o.fli[clean]).max() < (1e-2 if mode == 2 else 1e-3)
+    assert np.abs(g.fli.cpu().numpy()[clean] - o.fli[clean]).max() < (1e-2 if mode == 2 else FLI_VALUE_TOL)
 
 
 def test_batch_properties(mc):
@@ -505,7 +509,7 @@ def test_rk5_base_integrator_matches_oracle(mc):
         gc = I.integrate(w.states, 1.0, 1500, 3, shadow_eps=1e-8)
     o = oracle.integrate(w.states, 1.0, 1500, 3, shadow_eps=1e-8, integrator=oracle.RK5, **w.params())
     assert rel_state_err(g.states.cpu().numpy(), o.states) <= 4 * STATE_RTOL
-    assert np.abs(g.fli.cpu().numpy() - o.fli).max() < 1e-3
+    assert np.abs(g.fli.cpu().numpy() - o.fli).max() < FLI_VALUE_TOL
     assert np.array_equal(g.status.cpu().numpy(), o.status)
     assert np.array_equal(g.states.cpu().numpy(), gc.states.cpu().numpy())       # chunking: bit-identical
     assert np.array_equal(g.fli.cpu().numpy(), gc.fli.cpu().numpy())
@@ -710,7 +714,7 @@ def test_scan_command_line_tool(mc, tmp_path):
     assert head.startswith(b"P5\n314 1\n255\n")
     w = workloads.paper_scan_theta2(n_steps=600)
     o = oracle.integrate(w.states, 1.0, 600, 3, shadow_eps=1e-8, **w.params())
-    assert np.array_equal(z["status"], o.status & 255) and np.abs(z["fli"] - o.fli).max() < 1e-3
+    assert np.array_equal(z["status"], o.status & 255) and np.abs(z["fli"] - o.fli).max() < FLI_VALUE_TOL
 
 
 def test_config1_full_size_correction_on_and_off_in_the_same_run(mc):
@@ -852,7 +856,7 @@ def test_radiation_reaction_runs_match_oracle(mc, mode):
     if mode == 2:      # the dual scaling is singular twice per radial period (R7): bound on the bulk, loose cap on the worst orbit
         assert np.median(dfli) < 5e-3 and np.quantile(dfli, 0.9) < 5e-2 and dfli.max() < 0.5
     else:
-        assert dfli.max() < 2e-3
+        assert dfli.max() < FLI_VALUE_TOL
     W = ref[0] - ginv[0]
     G = ref[1:4] - ginv[1:4]
     assert (W < 0).all()                                                               # energy is radiated

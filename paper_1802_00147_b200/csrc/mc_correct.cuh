@@ -19,68 +19,93 @@ MC_DEV void references(const C& c, const T* z, RefsT<T>& R) {
   total_J(c, z, R.J0);
 }
 
-// Mode 3: minimal-norm Gauss-Newton projection of (r,p) onto {H = E0, r x p = J0 - S1 - S2}.
-// Constraint Jacobian rows: (a, b) = (dH/dr, dH/dp) and (p x e_k, e_k x r).  D D^T is
-//   [ g   c^T ]      g = a.a + b.b,  c = a x p + r x b,
-//   [ c   M   ]      M = (r.r + p.p) I - r r^T - p p^T
-// M^-1 is closed-form (Woodbury): M^-1 x = N(x)/D, D = (r.r + p.p) |L|^2,
-//   N(x) = |L|^2 x + r (rr (r.x) + rp (p.x)) + p (rp (r.x) + pp (p.x)),
-// so the 4x4 solve needs one reciprocal.  The oracle solves the same system by pivoted elimination.
+// Mode 3: minimal-norm Gauss-Newton projection of (r,p) onto {H = E0, r x p = Lt}, Lt = J0 - S1 - S2.
+// Constraint Jacobian D (4 x 6): row (a, b) = (dH/dr, dH/dp) and the three rows (p x e_k, e_k x r) of r x p.  The
+// step is d = D^T (D D^T)^-1 F, F = (H - E0, r x p - Lt), z <- z - d.  The oracle assembles D D^T and solves it by
+// pivoted elimination.  Here the same step is written out in the frame {r, p, L = r x p}:
+//   * the three L-rows have the null space N = span{n1 = (r, -p), n2 = (p, 0), n3 = (0, r)} (the deformations of
+//     (r, p) that keep r x p) and the row space {(p x l, l x r)}.  d = x + y, x in the row space, y in N.
+//   * x is fixed by the L-rows alone: M l = r x p - Lt, M = (r.r + p.p) I - r r^T - p p^T.  M maps r -> pp r - rp p,
+//     p -> rr p - rp r, L -> (rr + pp) L, so with l = lr r + lp p + lL L:  lr = -(Lt.r)/LL, lp = -(Lt.p)/LL,
+//     lL = (LL - Lt.L)/((rr + pp) LL), LL = |L|^2, and  p x l = -lr L + lL (pp r - rp p),  l x r = -lp L + lL (rr p - rp r).
+//   * y = g_N (f0 - g.x)/|g_N|^2, g_N the projection of g = (a, b) on N: g_N = sum_i alpha_i n_i, G alpha = beta,
+//     beta = (a.r - b.p, a.p, b.r), G = Gram matrix of n1..n3 = [[rr+pp, rp, -rp], [rp, pp, 0], [-rp, 0, rr]],
+//     det G = (rr + pp) LL, |g_N|^2 = beta.alpha.
+// So the step needs the gradient only through six dot products (with r, p, L), and those follow from the scalars of
+// the model routine without ever forming a and b (dH/dr = w1 s1 + w2 s2 + Cr r + B p + p x Sg, dH/dp = A p + B r +
+// Sg x r, Sg = u^3 (k1 sigma1 + k2 sigma2)):
+//   a.r = w1 a1 + w2 a2 + Cr rr + B rp + H_SO      b.p = A pp + B rp + H_SO
+//   a.p = w1 b1 + w2 b2 + Cr rp + B pp             b.r = A rp + B rr
+//   a.L = w1 l1 + w2 l2 + rp (Sg.p) - pp (Sg.r)    b.L = rp (Sg.r) - rr (Sg.p)
+// with a_i = sigma_i.r, b_i = sigma_i.p, l_i = sigma_i.L.  One reciprocal per step, no cross product besides L.
 //
-// gn_pass: ONE Gauss-Newton step on (r, p) = z[0:6] with the spins z[6:12] held fixed, towards energy E0 and orbital
-// angular momentum Lt = J0 - S1 - S2.  Returns whether another step is needed: |(dr,dp)|^2 > tol^2 p.p (R6;
-// PAPER.md:146, 197); false also for a non-finite step.
+// gn_pass: ONE Gauss-Newton step on (r, p) = z[0:6] with the spins z[6:12] held fixed.  Returns whether another step
+// is needed: |(dr,dp)|^2 > tol^2 p.p (R6); false also for a non-finite step.
 template <bool QM, class C, class T>
 MC_DEV bool gn_pass(const C& c, T* z, const T& E0, const T* Lt, double tol2) {
-  T g[12], H;
-  pn_eval<QM, false, true, false>(c, z, g, H);
   T* r = z;
   T* p = z + 3;
-  const T* a = g;
-  const T* b = g + 3;
-  T fL[3], cv[3];
-  cross3(r, p, fL);
-#pragma unroll
-  for (int i = 0; i < 3; ++i) fL[i] -= Lt[i];
+  const T* s1 = z + 6;
+  const T* s2 = z + 9;
+  OrbitalScalars<T> o;
+  orbital_scalars<true>(c, r, p, o);
+  const T rr = o.r2, pp = o.P, rp = o.rp, A = o.A, B = o.B;
+  T L[3];
+  cross3(r, p, L);
+  const T a1 = dot3(s1, r), a2 = dot3(s2, r);
+  const T b1 = dot3(s1, p), b2 = dot3(s2, p);
+  const T l1 = dot3(s1, L), l2 = dot3(s2, L);
+  const T k1u = c[K_K1] * o.u3, k2u = c[K_K2] * o.u3;
+  const T LS = fma(k2u, l2, k1u * l1);                 // H_SO = L.Sg
+  const T Sgr = fma(k2u, a2, k1u * a1);                // Sg.r
+  const T Sgp = fma(k2u, b2, k1u * b1);                // Sg.p
+  SpinScalars<T> q;
+  spin_scalars<QM, true>(c, s1, s2, o, a1, a2, LS, q);
+  const T Cr = o.u2 * fma(3.0, q.X, -o.Cu);
+  const T H = orbital_energy(c, o) + (LS + q.Hss);
   const T f0 = H - E0;
-  // c = a x p + r x b
-  cv[0] = fma(r[1], b[2], fma(-r[2], b[1], fma(a[1], p[2], -(a[2] * p[1]))));
-  cv[1] = fma(r[2], b[0], fma(-r[0], b[2], fma(a[2], p[0], -(a[0] * p[2]))));
-  cv[2] = fma(r[0], b[1], fma(-r[1], b[0], fma(a[0], p[1], -(a[1] * p[0]))));
-  const T gg = dot3(a, a) + dot3(b, b);
-  const T rr = dot3(r, r), pp = dot3(p, p), rp = dot3(r, p);
-  const T LL = fma(rr, pp, -(rp * rp));
-  const T D = (rr + pp) * LL;
-  // N(c), N(fL)
-  const T rc = dot3(r, cv), pc = dot3(p, cv), rf = dot3(r, fL), pf = dot3(p, fL);
-  const T cr_ = fma(rp, pc, rr * rc), cp_ = fma(pp, pc, rp * rc);
-  const T fr_ = fma(rp, pf, rr * rf), fp_ = fma(pp, pf, rp * rf);
-  T Nc[3], Nf[3];
-#pragma unroll
-  for (int i = 0; i < 3; ++i) {
-    Nc[i] = fma(p[i], cp_, fma(r[i], cr_, LL * cv[i]));
-    Nf[i] = fma(p[i], fp_, fma(r[i], fr_, LL * fL[i]));
-  }
-  const T S = fma(gg, D, -dot3(cv, Nc));
-  const T num = fma(D, f0, -dot3(cv, Nf));
-  const T DS = D * S;
-  const T inv = (DS != 0.0) ? rcp_nz(DS) : T(0.0);      // singular only for r || p or a circular orbit
-  const T l0 = num * D * inv;                         // num / S
-  const T sD = S * inv;                               // 1 / D
-  T lL[3], d1[3], d2[3];
-#pragma unroll
-  for (int i = 0; i < 3; ++i) lL[i] = fma(-l0, Nc[i], Nf[i]) * sD;
-  cross3(p, lL, d1);   // dr = l0 a + p x lL
-  cross3(lL, r, d2);   // dp = l0 b + lL x r
+  // the gradient's six dot products
+  const T t = fma(B, rp, LS);
+  const T ar = fma(q.w1, a1, fma(q.w2, a2, fma(Cr, rr, t)));
+  const T bp = fma(A, pp, t);
+  const T ap = fma(q.w1, b1, fma(q.w2, b2, fma(Cr, rp, B * pp)));
+  const T br = fma(A, rp, B * rr);
+  const T aL = fma(q.w1, l1, fma(q.w2, l2, fma(rp, Sgp, -(pp * Sgr))));
+  const T bL = fma(rp, Sgr, -(rr * Sgp));
+  // x: the L-rows
+  const T rp2 = rp * rp;
+  const T LL = fma(rr, pp, -rp2);
+  const T spp = rr + pp;
+  const T D = spp * LL;                                 // det G
+  const T mr = dot3(Lt, r), mp = dot3(Lt, p), nL = LL - dot3(Lt, L);   // lr = -mr/LL, lp = -mp/LL, lL = nL/D
+  // D (g.x) = (rr + pp)(mr a.L + mp b.L) + nL (pp a.r - rp (a.p + b.r) + rr b.p)
+  const T Dgx = fma(nL, fma(pp, ar, fma(rr, bp, -(rp * (ap + br)))), spp * fma(mr, aL, mp * bL));
+  // y: D alpha = adj(G) beta, T = D |g_N|^2
+  const T be1 = ar - bp;
+  const T C12 = -(rp * rr), C13 = rp * pp;
+  const T al1 = fma(rr * pp, be1, fma(C12, ap, C13 * br));
+  const T al2 = fma(C12, be1, fma(fma(rr, rr, LL), ap, -(rp2 * br)));
+  const T al3 = fma(C13, be1, fma(fma(pp, pp, LL), br, -(rp2 * ap)));
+  const T Tn = fma(be1, al1, fma(ap, al2, br * al3));
+  const T TD = Tn * D;
+  const T inv = (TD != 0.0) ? rcp_nz(TD) : T(0.0);     // singular only for r || p or a circular orbit: zero step
+  const T invD = Tn * inv;
+  const T sy = fma(f0, D, -Dgx) * inv;                  // (f0 - g.x) / (D |g_N|^2)
+  const T lL = nL * invD;
+  const T iLL = spp * invD;                             // 1 / LL
+  const T y1 = sy * al1, lLrp = lL * rp;
+  const T crr = fma(lL, pp, y1), crp = fma(sy, al2, -lLrp), crL = mr * iLL;      // dr = crr r + crp p + crL L
+  const T cpr = fma(sy, al3, -lLrp), cpp = fma(lL, rr, -y1), cpL = mp * iLL;     // dp = cpr r + cpp p + cpL L
   T dd = 0.0;
+  T dr[3], dp[3];
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
-    const T dr = fma(l0, a[i], d1[i]);
-    const T dp = fma(l0, b[i], d2[i]);
-    dd = fma(dr, dr, fma(dp, dp, dd));
-    r[i] -= dr;
-    p[i] -= dp;
+    dr[i] = fma(crr, r[i], fma(crp, p[i], crL * L[i]));
+    dp[i] = fma(cpr, r[i], fma(cpp, p[i], cpL * L[i]));
+    dd = fma(dr[i], dr[i], fma(dp[i], dp[i], dd));
   }
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { r[i] -= dr[i]; p[i] -= dp[i]; }
   return dd > tol2 * pp;
 }
 

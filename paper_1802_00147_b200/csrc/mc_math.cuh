@@ -99,6 +99,78 @@ MC_DEV void cross3(const T* a, const T* b, T* c) {
 }
 
 // ---- the fused model routine ----------------------------------------------------------------------
+// Scalars of the orbital part (N + 1PN + 2PN) at one point: everything is a polynomial in P = p.p, Q = (n.p)^2 and
+// u = 1/|r| (Horner; every constant multiple is precomputed, mc_consts.h).
+//   dH_orb/dp = A p + B r,   dH_orb/dr = B p - u^2 Cu r
+template <class T>
+struct OrbitalScalars { T r2, u, u2, u3, u5, rp, P, w, Q, t1, t2, t3, A, B, Cu; };
+
+template <bool WANT_H, class C, class T>
+MC_DEV void orbital_scalars(const C& c, const T* r, const T* p, OrbitalScalars<T>& o) {
+  o.r2 = dot3(r, r);
+  o.u = rsqrt_pos(o.r2);
+  o.u2 = o.u * o.u; o.u3 = o.u2 * o.u; o.u5 = o.u3 * o.u2;
+  o.rp = dot3(r, p);
+  o.P = dot3(p, p);
+  o.w = o.rp * o.u2;                                          // (n.p) u
+  o.Q = o.rp * o.w;                                           // (n.p)^2
+  const T u = o.u, P = o.P, Q = o.Q;
+  o.t1 = fma(c[K_D2], Q, fma(c[K_D1], P, c[K_B1]));           // b1 + d1 P + d2 Q
+  o.t2 = fma(c[K_D3], Q, c[K_B2]);                            // b2 + d3 Q
+  o.t3 = WANT_H ? fma(c[K_E2], Q, c[K_E1] * P) : T(0.0);      // e1 P + e2 Q (only H itself needs it)
+  // H_P = 1/2 + P (2 a1 + 3 c3 P) + u (b1 + 2 d1 P + d2 Q + e1 u)
+  const T hp_u = fma(c[K_E1], u, fma(c[K_D1], P, o.t1));
+  const T HP = fma(u, hp_u, fma(P, fma(c[K_3C3], P, c[K_2A1]), 0.5));
+  // 2 H_Q = u (2 b2 + 2 d2 P + 4 d3 Q + 2 e2 u)
+  const T HQ2 = u * fma(c[K_4D3], Q, fma(c[K_2D2], P, fma(c[K_2E2], u, c[K_2B2])));
+  // H_u = -1 + P t1 + Q t2 + u (2 h1 + 2 t3 + 3 f1 u)
+  const T hu_u = WANT_H ? fma(c[K_3F1], u, fma(2.0, o.t3, c[K_2H1]))
+                        : fma(c[K_3F1], u, fma(c[K_2E1], P, fma(c[K_2E2], Q, c[K_2H1])));
+  const T Hu = fma(u, hu_u, fma(Q, o.t2, fma(P, o.t1, -1.0)));
+  o.A = HP + HP;
+  o.B = HQ2 * o.w;
+  o.Cu = fma(Hu, u, HQ2 * Q);
+}
+
+// H_orb = P/2 - u + P^2 (a1 + c3 P) + u (P t1 + Q t2) + u^2 (h1 + t3) + f1 u^3
+template <class C, class T>
+MC_DEV T orbital_energy(const C& c, const OrbitalScalars<T>& o) {
+  return fma(o.u2, fma(c[K_F1], o.u, c[K_H1] + o.t3),
+             fma(o.u, fma(o.Q, o.t2, o.P * o.t1), fma(o.P * o.P, fma(c[K_C3], o.P, c[K_A1]), fma(0.5, o.P, -o.u))));
+}
+
+// Spin-spin (and quadrupole-monopole) scalars from a_i = sigma_i.r, d_ij = sigma_i.sigma_j and LS = H_SO:
+//   X:  the coefficient of r in dH_spin/dr is 3 u^2 X,  X = -H_SO + c12 (d12 u^3 - 5 a1 a2 u^5) + QM
+//   w_i: the coefficient of sigma_i in dH_spin/dr;  Hss = H_12 + H_11 + H_22 (WANT_H)
+template <class T>
+struct SpinScalars { T X, w1, w2, Hss; };
+
+template <bool QM, bool WANT_H, class C, class T>
+MC_DEV void spin_scalars(const C& c, const T* s1, const T* s2, const OrbitalScalars<T>& o, const T& a1, const T& a2,
+                         const T& LS, SpinScalars<T>& q) {
+  const T d12 = dot3(s1, s2);
+  const T a12u5 = a1 * a2 * o.u5;
+  const T c12u3 = c[K_C12] * o.u3;
+  q.X = fma(c12u3, d12, fma(c[K_M5C12], a12u5, -LS));
+  const T c12u5x3 = c[K_3C12] * o.u5;
+  q.w1 = c12u5x3 * a2;
+  q.w2 = c12u5x3 * a1;
+  q.Hss = fma(c[K_3C12], a12u5, -(c12u3 * d12));
+  if (QM) {
+    // H_ii = q_i (3 a_i^2 u^5 - d_ii u^3).  Only q_i itself is used as a constant (no multiples), so that the
+    // per-orbit-kappa variant keeps one register per body; the numeric factors ride as FMA immediates.
+    const T d11 = dot3(s1, s1), d22 = dot3(s2, s2);
+    const T q1u3 = c[K_Q1] * o.u3, q2u3 = c[K_Q2] * o.u3;
+    const T q1a = q1u3 * o.u2 * a1, q2a = q2u3 * o.u2 * a2;    // q_i u^5 a_i
+    const T q1aa = q1a * a1, q2aa = q2a * a2;                  // q_i u^5 a_i^2
+    q.X = fma(q1u3, d11, fma(-5.0, q1aa, q.X));
+    q.X = fma(q2u3, d22, fma(-5.0, q2aa, q.X));
+    q.w1 = fma(6.0, q1a, q.w1);
+    q.w2 = fma(6.0, q2a, q.w2);
+    if (WANT_H) q.Hss += fma(3.0, q1aa, -(q1u3 * d11)) + fma(3.0, q2aa, -(q2u3 * d22));
+  }
+}
+
 // Input  z = (r[0:3], p[3:6], sigma1[6:9], sigma2[9:12]).
 // Output g[0:3] = dH/dr, g[3:6] = dH/dp; if OMEGA: g[6:9] = Omega1, g[9:12] = Omega2; if WANT_H: H.
 // With RR (2.5PN radiation reaction, MC_TERM_RR; only the equations of motion use it): g[0:3] = dH/dr - F, so that
@@ -112,33 +184,12 @@ MC_DEV void pn_eval(const C& c, const T* z, T* g, T& H) {
   const T* p = z + 3;
   const T* s1 = z + 6;
   const T* s2 = z + 9;
-  const T r2 = dot3(r, r);
-  const T u = rsqrt_pos(r2);
-  const T u2 = u * u, u3 = u2 * u, u5 = u3 * u2;
-  const T rp = dot3(r, p);
-  const T P = dot3(p, p);
-  const T w = rp * u2;                                        // (n.p) u
-  const T Q = rp * w;                                         // (n.p)^2
-
-  // orbital polynomials (Horner); every constant multiple is precomputed (mc_consts.h)
-  const T t1 = fma(c[K_D2], Q, fma(c[K_D1], P, c[K_B1]));   // b1 + d1 P + d2 Q
-  const T t2 = fma(c[K_D3], Q, c[K_B2]);                    // b2 + d3 Q
-  const T t3 = WANT_H ? fma(c[K_E2], Q, c[K_E1] * P) : T(0.0);  // e1 P + e2 Q (only H itself needs it)
-  // H_P = 1/2 + P (2 a1 + 3 c3 P) + u (b1 + 2 d1 P + d2 Q + e1 u)
-  const T hp_u = fma(c[K_E1], u, fma(c[K_D1], P, t1));
-  const T HP = fma(u, hp_u, fma(P, fma(c[K_3C3], P, c[K_2A1]), 0.5));
-  // 2 H_Q = u (2 b2 + 2 d2 P + 4 d3 Q + 2 e2 u)
-  const T HQ2 = u * fma(c[K_4D3], Q, fma(c[K_2D2], P, fma(c[K_2E2], u, c[K_2B2])));
-  // H_u = -1 + P t1 + Q t2 + u (2 h1 + 2 t3 + 3 f1 u)
-  const T hu_u = WANT_H ? fma(c[K_3F1], u, fma(2.0, t3, c[K_2H1]))
-                        : fma(c[K_3F1], u, fma(c[K_2E1], P, fma(c[K_2E2], Q, c[K_2H1])));
-  const T Hu = fma(u, hu_u, fma(Q, t2, fma(P, t1, -1.0)));
-  const T A = HP + HP;                                // dH_orb/dp = A p + B r
-  const T B = HQ2 * w;
-  const T Cu = fma(Hu, u, HQ2 * Q);                   // dH_orb/dr = B p - u^2 Cu r
+  OrbitalScalars<T> o;
+  orbital_scalars<WANT_H>(c, r, p, o);
+  const T u2 = o.u2, u3 = o.u3, u5 = o.u5, A = o.A, B = o.B;
 
   // spin couplings
-  const T a1 = dot3(s1, r), a2 = dot3(s2, r), d12 = dot3(s1, s2);
+  const T a1 = dot3(s1, r), a2 = dot3(s2, r);
   const T k1u = c[K_K1] * u3, k2u = c[K_K2] * u3;
   T Sg[3], L[3], SxR[3], PxS[3];
 #pragma unroll
@@ -147,41 +198,23 @@ MC_DEV void pn_eval(const C& c, const T* z, T* g, T& H) {
   cross3(Sg, r, SxR);
   cross3(p, Sg, PxS);
   const T LS = dot3(L, Sg);                                      // = H_SO
-  const T a12u5 = a1 * a2 * u5;
-  const T c12u3 = c[K_C12] * u3;
-  // coefficient of r in dH_spin/dr is 3 u^2 X:  X = -H_SO + c12 (d12 u^3 - 5 a1 a2 u^5) + QM
-  T X = fma(c12u3, d12, fma(c[K_M5C12], a12u5, -LS));
-  const T c12u5x3 = c[K_3C12] * u5;
-  T w1 = c12u5x3 * a2, w2 = c12u5x3 * a1;
-  T Hss = fma(c[K_3C12], a12u5, -(c12u3 * d12));
-  if (QM) {
-    // H_ii = q_i (3 a_i^2 u^5 - d_ii u^3).  Only q_i itself is used as a constant (no multiples), so that the
-    // per-orbit-kappa variant keeps one register per body; the numeric factors ride as FMA immediates.
-    const T d11 = dot3(s1, s1), d22 = dot3(s2, s2);
-    const T q1u3 = c[K_Q1] * u3, q2u3 = c[K_Q2] * u3;
-    const T q1a = q1u3 * u2 * a1, q2a = q2u3 * u2 * a2;        // q_i u^5 a_i
-    const T q1aa = q1a * a1, q2aa = q2a * a2;                  // q_i u^5 a_i^2
-    X = fma(q1u3, d11, fma(-5.0, q1aa, X));
-    X = fma(q2u3, d22, fma(-5.0, q2aa, X));
-    w1 = fma(6.0, q1a, w1);
-    w2 = fma(6.0, q2a, w2);
-    if (WANT_H) Hss += fma(3.0, q1aa, -(q1u3 * d11)) + fma(3.0, q2aa, -(q2u3 * d22));
-  }
-  T Cr = u2 * fma(3.0, X, -Cu);                       // coefficient of r in dH/dr
+  SpinScalars<T> q;
+  spin_scalars<QM, WANT_H>(c, s1, s2, o, a1, a2, LS, q);
+  T Cr = u2 * fma(3.0, q.X, -o.Cu);                   // coefficient of r in dH/dr
   T Bp = B;                                           // coefficient of p in dH/dr
   if constexpr (RR) {
-    const T ca = fma(c[K_RA3], Q, fma(c[K_RA2], u, c[K_RA1] * P));
-    const T cb = fma(c[K_RB3], Q, fma(c[K_RB2], u, c[K_RB1] * P));
-    const T fr = ca * w * u3, fp = -(cb * u3);         // F = fr r + fp p
+    const T ca = fma(c[K_RA3], o.Q, fma(c[K_RA2], o.u, c[K_RA1] * o.P));
+    const T cb = fma(c[K_RB3], o.Q, fma(c[K_RB2], o.u, c[K_RB1] * o.P));
+    const T fr = ca * o.w * u3, fp = -(cb * u3);       // F = fr r + fp p
     Cr -= fr;
     Bp -= fp;
-    g[12] = fma(fr, fma(A, rp, B * r2), fp * fma(A, P, fma(B, rp, LS)));
+    g[12] = fma(fr, fma(A, o.rp, B * o.r2), fp * fma(A, o.P, fma(B, o.rp, LS)));
 #pragma unroll
     for (int i = 0; i < 3; ++i) g[13 + i] = fp * L[i];
   }
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
-    g[i] = fma(w2, s2[i], fma(w1, s1[i], fma(Cr, r[i], fma(Bp, p[i], PxS[i]))));
+    g[i] = fma(q.w2, s2[i], fma(q.w1, s1[i], fma(Cr, r[i], fma(Bp, p[i], PxS[i]))));
     g[3 + i] = fma(A, p[i], fma(B, r[i], SxR[i]));
   }
   if (OMEGA) {
@@ -197,11 +230,7 @@ MC_DEV void pn_eval(const C& c, const T* z, T* g, T& H) {
       g[9 + i] = fma(-m21u, s1[i], fma(b2r, r[i], o2u * L[i]));
     }
   }
-  if (WANT_H) {
-    // H = P/2 - u + P^2 (a1 + c3 P) + u (P t1 + Q t2) + u^2 (h1 + t3) + f1 u^3 + H_SO + H_SS
-    const T orb = fma(u2, fma(c[K_F1], u, c[K_H1] + t3), fma(u, fma(Q, t2, P * t1), fma(P * P, fma(c[K_C3], P, c[K_A1]), fma(0.5, P, -u))));
-    H = orb + (LS + Hss);
-  }
+  if (WANT_H) H = orbital_energy(c, o) + (LS + q.Hss);
 }
 
 // dz/dt, eqs (6)-(7): dr/dt = dH/dp, dp/dt = -dH/dr (+ a_2.5PN), dsigma_i/dt = Omega_i x sigma_i.

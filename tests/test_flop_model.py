@@ -35,7 +35,7 @@ def test_terms_and_modes_add_what_they_should():
     assert m1["correct_fixed"] == dict(fma=4, mul=8, add=0, special=2, flop=18)       # eq (10) twice: dot, rsqrt, 3 mul
     assert base["correct_fixed"]["flop"] == 18 + 12                                   # + L_t = J0 - s1 S1 - s2 S2
     assert m2["gn_step"]["flop"] == 0 and 200 < m2["correct_fixed"]["flop"] < 400      # polynomial dual scaling (SURVEY: ~0.3 k)
-    assert 350 < base["gn_step"]["flop"] < 450 and base["gn_step"]["special"] == 2     # one rsqrt (eval) + one reciprocal (solve)
+    assert 280 < base["gn_step"]["flop"] < 350 and base["gn_step"]["special"] == 2     # one rsqrt (eval) + one reciprocal (solve); 395 before the step was written in the {r, p, L} frame
     assert base["status"]["flop"] == 5
     it2, it6 = binding.flop_model(15, 2, RK4, 2), binding.flop_model(15, 2, RK4, 6)
     per_iter = (it6["correct_fixed"]["flop"] - it2["correct_fixed"]["flop"]) / 4

@@ -43,7 +43,7 @@ enum mc_terms {
                          carries the work W = int (dr/dt).a dt and the torque integral G = int r x a dt of the
                          force, and the correction (modes 2, 3) targets E0 + W and J0 + G, the "integral invariant
                          relation" of PAPER.md:221; see mc_get_dissipation.  Default off.  One combination is not
-                         built: per_orbit = 1 together with MC_INTEG_RK5 (mc_integrate returns MC_EINVAL; the 45
+                         built: per_orbit = 1 together with MC_INTEG_RK5 (mc_integrate, and mc_eval with what = 3, return MC_EINVAL; the 45
                          per-orbit constants, six stages and 16 components exceed the 255-register budget and the
                          library ships no kernel that spills)                                               */
 };
@@ -225,7 +225,8 @@ int mc_debug_check(mc_handle* h, int64_t* out_line);
  *             out[16][n], rows 12-15 = dW/dt, dG/dt
  *   what = 2: out[6][n]  = E, Jx, Jy, Jz, |S1hat|, |S2hat|
  *   what = 3: out[12][n] = one step of the base integrator (params.integrator) of size step_h, no correction;
- *             with MC_TERM_RR out[16][n], rows 12-15 = W, G accumulated over the step (from zero)
+ *             with MC_TERM_RR out[16][n], rows 12-15 = W, G accumulated over the step (from zero); MC_EINVAL for the one
+ *             combination that is not built (per_orbit = 1, MC_INTEG_RK5, MC_TERM_RR; see MC_TERM_RR)
  *   what = 4: out[12][n] = correction operator of mode `mode` applied to states, with references
  *             refs = DEVICE double[4][n] (E0, J0x, J0y, J0z); required for every mode (MC_EINVAL if NULL)
  * Asynchronous on the handle's stream. */

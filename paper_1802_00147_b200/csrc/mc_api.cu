@@ -99,8 +99,14 @@ eval_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ mc::Int
     rows = 6;
   } else if (what == 3) {
     if (rr) {
-      if (A.integrator == 1) mc::rk5_step<QM, true>(c, z, A.hw, f);
-      else mc::rk4_step<QM, true>(c, z, A.hw, f);
+      // fully per-orbit parameters + RK5 + 2.5PN is the one combination that is not built (register budget;
+      // mc_integrate and mc_eval return MC_EINVAL for it)
+      if constexpr (PARAMS != mc::PARAMS_PER_ORBIT) {
+        if (A.integrator == 1) mc::rk5_step<QM, true>(c, z, A.hw, f);
+        else mc::rk4_step<QM, true>(c, z, A.hw, f);
+      } else {
+        mc::rk4_step<QM, true>(c, z, A.hw, f);
+      }
       rows = 16;
     } else if (A.integrator == 1) mc::rk5_step<QM, false>(c, z, A.hw, f);
     else mc::rk4_step<QM, false>(c, z, A.hw, f);
@@ -528,6 +534,7 @@ int mc_eval(mc_handle* h, int32_t what, const double* states, int64_t n, double 
   if (n == 0) return MC_OK;
   if (!states || !out) return MC_EINVAL;
   if (what == 4 && (mode < 0 || mode > 3 || !refs)) return MC_EINVAL;   // the kernel reads refs for every mode
+  if (what == 3 && h->P.per_orbit == 1 && h->P.integrator == 1 && (h->P.terms & MC_TERM_RR)) return MC_EINVAL;   // not built
   MC_CUDA(cudaSetDevice(h->P.device));
   mc::IntegrateArgs A;
   fill_args(h, A);

@@ -60,7 +60,7 @@ MC_DEV bool gn_pass(const C& c, T* z, const T& E0, const T* Lt, double tol2) {
   const T Sgr = fma(k2u, a2, k1u * a1);                // Sg.r
   const T Sgp = fma(k2u, b2, k1u * b1);                // Sg.p
   SpinScalars<T> q;
-  spin_scalars<QM, true>(c, s1, s2, o, a1, a2, LS, q);
+  spin_scalars<QM, true>(c, s1, s2, o, a1, a2, o.u5 * a1, o.u5 * a2, LS, q);
   const T Cr = o.u2 * fma(3.0, q.X, -o.Cu);
   const T H = orbital_energy(c, o) + (LS + q.Hss);
   const T f0 = H - E0;

@@ -147,21 +147,20 @@ struct SpinScalars { T X, w1, w2, Hss; };
 
 template <bool QM, bool WANT_H, class C, class T>
 MC_DEV void spin_scalars(const C& c, const T* s1, const T* s2, const OrbitalScalars<T>& o, const T& a1, const T& a2,
-                         const T& LS, SpinScalars<T>& q) {
+                         const T& ua1, const T& ua2 /* u^5 a_i */, const T& LS, SpinScalars<T>& q) {
   const T d12 = dot3(s1, s2);
-  const T a12u5 = a1 * a2 * o.u5;
+  const T a12u5 = a1 * ua2;
   const T c12u3 = c[K_C12] * o.u3;
   q.X = fma(c12u3, d12, fma(c[K_M5C12], a12u5, -LS));
-  const T c12u5x3 = c[K_3C12] * o.u5;
-  q.w1 = c12u5x3 * a2;
-  q.w2 = c12u5x3 * a1;
+  q.w1 = c[K_3C12] * ua2;
+  q.w2 = c[K_3C12] * ua1;
   q.Hss = fma(c[K_3C12], a12u5, -(c12u3 * d12));
   if (QM) {
     // H_ii = q_i (3 a_i^2 u^5 - d_ii u^3).  Only q_i itself is used as a constant (no multiples), so that the
     // per-orbit-kappa variant keeps one register per body; the numeric factors ride as FMA immediates.
     const T d11 = dot3(s1, s1), d22 = dot3(s2, s2);
     const T q1u3 = c[K_Q1] * o.u3, q2u3 = c[K_Q2] * o.u3;
-    const T q1a = q1u3 * o.u2 * a1, q2a = q2u3 * o.u2 * a2;    // q_i u^5 a_i
+    const T q1a = c[K_Q1] * ua1, q2a = c[K_Q2] * ua2;          // q_i u^5 a_i
     const T q1aa = q1a * a1, q2aa = q2a * a2;                  // q_i u^5 a_i^2
     q.X = fma(q1u3, d11, fma(-5.0, q1aa, q.X));
     q.X = fma(q2u3, d22, fma(-5.0, q2aa, q.X));
@@ -190,6 +189,7 @@ MC_DEV void pn_eval(const C& c, const T* z, T* g, T& H) {
 
   // spin couplings
   const T a1 = dot3(s1, r), a2 = dot3(s2, r);
+  const T ua1 = u5 * a1, ua2 = u5 * a2;                               // every a_i that meets u^5 does so through these
   const T k1u = c[K_K1] * u3, k2u = c[K_K2] * u3;
   T Sg[3], L[3], SxR[3], PxS[3];
 #pragma unroll
@@ -199,7 +199,7 @@ MC_DEV void pn_eval(const C& c, const T* z, T* g, T& H) {
   cross3(p, Sg, PxS);
   const T LS = dot3(L, Sg);                                      // = H_SO
   SpinScalars<T> q;
-  spin_scalars<QM, WANT_H>(c, s1, s2, o, a1, a2, LS, q);
+  spin_scalars<QM, WANT_H>(c, s1, s2, o, a1, a2, ua1, ua2, LS, q);
   T Cr = u2 * fma(3.0, q.X, -o.Cu);                   // coefficient of r in dH/dr
   T Bp = B;                                           // coefficient of p in dH/dr
   if constexpr (RR) {
@@ -220,10 +220,8 @@ MC_DEV void pn_eval(const C& c, const T* z, T* g, T& H) {
   if (OMEGA) {
     const T o1u = c[K_O1] * u3, o2u = c[K_O2] * u3;
     const T m12u = c[K_M12] * u3, m21u = c[K_M21] * u3;
-    T b1r = c[K_3M12] * a2, b2r = c[K_3M21] * a1;
-    if (QM) { b1r = fma(c[K_3M11], a1, b1r); b2r = fma(c[K_3M22], a2, b2r); }
-    b1r *= u5;
-    b2r *= u5;
+    T b1r = c[K_3M12] * ua2, b2r = c[K_3M21] * ua1;             // 3 u^5 (m12 a2 + m11 a1), 3 u^5 (m21 a1 + m22 a2)
+    if (QM) { b1r = fma(c[K_3M11], ua1, b1r); b2r = fma(c[K_3M22], ua2, b2r); }
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
       g[6 + i] = fma(-m12u, s2[i], fma(b1r, r[i], o1u * L[i]));

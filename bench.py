@@ -34,7 +34,7 @@ UNIT = "orbit-steps/s"
 # dram__bytes_read.sum + dram__bytes_write.sum from the ncu capture of that very launch configuration
 # (profiles/r02_ncu_integrate_kernel_mode3.md, section "DRAM traffic of the full-length launch").  Outputs (31 MB) and the carry buffer (31 MB) live in the 126 MB L2;
 # algorithmic: 340 B per orbit.
-NCU_DRAM_BYTES_PER_LAUNCH_314 = 10183168 + 7404544   # read + write, bytes
+NCU_DRAM_BYTES_PER_LAUNCH_314 = 10028800 + 7679232   # read + write, bytes
 FP64_LANES_PER_SM = 64
 
 

@@ -113,6 +113,38 @@ def test_correction_operator_matches_oracle(mc, mode, terms):
     assert drift(got, I0, terms=terms, **par) < (1e-14 if mode == 3 else 1.0)
 
 
+def test_mode3_operator_near_the_circular_singularity(mc):
+    """The degenerate case of mode 3: for a circular orbit the energy row of the constraint
+    Jacobian is a combination of the angular-momentum rows and the projection is singular; for a nearly circular one it
+    is ill conditioned like 1/e^2.  Newtonian Hamiltonian (terms = 0), BASELINE config 0's initial conditions, which
+    reach p_y = 0.99993 of the circular value.  Bars: the bulk agrees with the long-double oracle to round-off; the
+    worst orbit of ONE Gauss-Newton step to 1e-8 -- and the kernel's closed form in the frame {r, p, L} stays closer to
+    the long-double result than the oracle's own double instance (pivoted elimination in FP64: 2.5e-7 on the same
+    input), which is what an ill-conditioned solve costs in double precision.  (Measured: 6.5e-11 / 7e-12 for one
+    step, 1.6e-8 / 1.6e-9 for the epsilon-terminated iteration, beta = 0.8 / 0.1.)"""
+    w = workloads.config0(257)
+    r0 = np.linalg.norm(w.states[0:3], axis=0)
+    assert (np.linalg.norm(w.states[3:6], axis=0) * np.sqrt(r0)).max() > 0.9999      # the input does contain the near-circular orbit
+    rng = np.random.default_rng(5)
+    zp = w.states * (1 + 1e-6 * rng.normal(size=w.states.shape))
+    for beta in (0.8, 0.1):
+        par = dict(beta=beta, chi1=1.0, chi2=0.0)
+        I0 = oracle.integrals(w.states, terms=0, **par)
+        for iters, cap in ((1, 1e-8), (4, 1e-6)):
+            want, _ = oracle.correct(zp, I0[0], I0[1:4], 3, terms=0, newton_iters=iters, **par)
+            want_double, _ = oracle.correct(zp, I0[0], I0[1:4], 3, terms=0, newton_iters=iters, precision=oracle.DOUBLE, **par)
+            with mc.Integrator(terms=0, newton_iters=iters, **par) as I:
+                got = I.eval("correct", zp, mode=3, refs=I0[0:4]).cpu().numpy()
+
+            def per_orbit(a):
+                return np.max([np.linalg.norm(a[s] - want[s], axis=0) / np.linalg.norm(want[s], axis=0)
+                               for s in (slice(0, 3), slice(3, 6))], axis=0)
+            e_gpu, e_double = per_orbit(got), per_orbit(want_double)
+            assert np.median(e_gpu) < 1e-14
+            assert e_gpu.max() < cap
+            assert e_double.max() > 1e-8 and e_gpu.max() < e_double.max()
+
+
 def test_config0_state_parity_after_1e3_steps_and_drift_after_1e4(mc):
     """BASELINE config 0: 64 orbits, mode 3, no shadow."""
     w = workloads.config0()

@@ -113,6 +113,24 @@ def test_correction_operator_matches_oracle(mc, mode, terms):
     assert drift(got, I0, terms=terms, **par) < (1e-14 if mode == 3 else 1.0)
 
 
+def test_plain_c_program_drives_the_library(mc, tmp_path):
+    """The boundary is a C ABI: tests/c_abi_caller.c (C99, no Python, no torch, no CUDA headers) is compiled with gcc
+    against include/mc.h, linked with libmc.so and run; it integrates 40 shadowed orbits through mc_integrate_host and
+    checks return codes, status, drift of the integrals <= 1e-12, FLI range, zero spills and run-to-run bit identity."""
+    import os
+    import subprocess
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    mc.load_library()                                     # builds libmc.so if it is stale
+    pkg = os.path.join(root, "paper_1802_00147_b200")
+    exe = str(tmp_path / "c_abi_caller")
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-O1", "-I", os.path.join(root, "include"),
+                    os.path.join(root, "tests", "c_abi_caller.c"), "-o", exe, "-L", pkg, "-l:libmc.so",
+                    "-Wl,-rpath," + pkg, "-lm"], check=True)
+    r = subprocess.run([exe], capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert "c_abi_caller ok" in r.stdout
+
+
 def test_mode3_operator_near_the_circular_singularity(mc):
     """The degenerate case of mode 3: for a circular orbit the energy row of the constraint
     Jacobian is a combination of the angular-momentum rows and the projection is singular; for a nearly circular one it

@@ -58,9 +58,20 @@ def build(force: bool = False, verbose: bool = False, checked: bool = False) -> 
     if not checked and not force and not is_stale():
         return LIB
     obj_dir = OBJ + ("_checked" if checked else "")
+    os.makedirs(obj_dir, exist_ok=True)
+    # one builder at a time: under torchrun every rank imports the binding, and if the library is stale they would
+    # all compile into the same object files.  The others wait here and then find a fresh library.
+    import fcntl
+    with open(os.path.join(obj_dir, ".lock"), "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        if not checked and not force and not is_stale():
+            return LIB
+        return _build_locked(obj_dir, verbose, checked)
+
+
+def _build_locked(obj_dir: str, verbose: bool, checked: bool) -> str:
     lib = LIB_CHECKED if checked else LIB
     flags = NVCC_FLAGS + (["-DMC_CHECKED"] if checked else [])
-    os.makedirs(obj_dir, exist_ok=True)
     nvcc = os.environ.get("NVCC", "nvcc")
 
     def compile_one(src):

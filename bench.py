@@ -47,7 +47,7 @@ def parse_args():
     ap.add_argument("--grid", type=int, default=314, help="grid edge (314 = BASELINE config 2)")
     ap.add_argument("--n-steps", type=int, default=None, help="RK4 steps per orbit (default: the workload's own; 1e5 for config 2)")
     ap.add_argument("--workload", default="config2",
-                    help="config2 (default, the bench line) | config0 | config1 | config1:mode0 | config3 | config3:qmoff | "
+                    help="config2 (default, the bench line) | config2:rr | config0 | config1 | config1:mode0 | config3 | config3:qmoff | "
                          "config4:<log2 n> | paper-theta2 | paper-theta2:0 | paper-plane  -- the other BASELINE configs and the "
                          "paper's own scans (PAPER.md:227), for profiles/ tables only")
     ap.add_argument("--integrator", default="rk4", choices=["rk4", "rk5"],
@@ -163,7 +163,10 @@ def global_workload(args, world):
     name, _, opt = args.workload.partition(":")
     kw = {} if args.n_steps is None else {"n_steps": args.n_steps}
     if name == "config2":
-        return workloads.config2(n_r=args.grid * world, n_theta=args.grid, **kw)
+        w = workloads.config2(n_r=args.grid * world, n_theta=args.grid, **kw)
+        if opt == "rr":                             # the same scan with the 2.5PN radiation reaction (MC_TERM_RR)
+            w.terms |= 32
+        return w
     if name == "config0":
         return workloads.config0(**kw)
     if name == "config1":
@@ -192,7 +195,7 @@ def describe(w, args):
     integ = "RK5 (Butcher six-stage)" if args.integrator == "rk5" else "RK4"
     if w.name.startswith("config2"):
         return (f"config2: {args.grid}x{args.grid} orbit scan per GPU (r0 in [10,60] x theta in [0,pi]), equal mass, chi=1, "
-                f"N+1PN+2PN+SO+SS, {integ} h=1, {w.n_steps} steps, shadow 1e-8 renormalised every 100 steps + FLI, "
+                f"N+1PN+2PN+SO+SS{'+2.5PN radiation reaction' if w.terms & 32 else ''}, {integ} h=1, {w.n_steps} steps, shadow 1e-8 renormalised every 100 steps + FLI, "
                 + ("six-integral correction (mode 3, Gauss-Newton terminated at eps=1e-10, cap 4)" if w.correction_mode == 3
                    else f"correction mode {w.correction_mode}"))
     return (f"{args.workload} ({w.name}): {w.n_orbits} orbits per GPU, terms mask {w.terms}, "

@@ -28,7 +28,8 @@ enum mc_error {
   MC_EINVAL = -1,  /* null pointer, negative size, unknown mode/term bit, beta outside (0,1], ... */
   MC_ECUDA = -2,   /* a CUDA runtime call failed; mc_strerror(MC_ECUDA) returns the CUDA message  */
   MC_EARCH = -3,   /* the device is not compute capability 10.x (the library holds sm_100a code only) */
-  MC_ENOMEM = -4   /* host allocation failed */
+  MC_ENOMEM = -4,  /* host allocation failed */
+  MC_ELIMIT = -5   /* mc_integrate_static only: the batch exceeds MC_STATIC_MAX_TRAJECTORIES */
 };
 
 /* Hamiltonian terms, eq (1) of the paper.  H_N is always on. */
@@ -185,6 +186,46 @@ int mc_integrate_ex(mc_handle* h, const double* states, int64_t n_orbits, double
 int mc_integrate_host(mc_handle* h, const double* states, int64_t n_orbits, double step_h,
                       int64_t n_steps, int32_t correction_mode, double shadow_eps, double* out_states,
                       double* out_invariants, double* out_fli, int32_t* out_status, int64_t* out_step);
+
+/* mc_integrate for callers that must not allocate device memory.
+ *
+ * Why it exists.  A handle gets its device bookkeeping (work queue of the persistent kernel, per-orbit Gauss-Newton
+ * counters, status arrays) from cudaMalloc, on first use and again whenever a batch is larger than any before.  That
+ * is unusable for a program that has handed the whole GPU to its own memory pool (a later cudaMalloc by a library
+ * just fails), for a loop with a latency budget (cudaMalloc / cudaFree stall all streams of the process), and
+ * wherever the runtime refuses allocation outright, e.g. while a stream of the process is being captured.  This
+ * entry point needs no handle and calls neither cudaMalloc nor cudaFree nor any library routine that allocates: its
+ * bookkeeping lives in a fixed array compiled into libmc.so (256 bytes + 8 bytes x MC_STATIC_MAX_TRAJECTORIES, about
+ * 256 KB).  Every GPU on which the library's code is loaded holds that array until the process exits, used or not.
+ *
+ * Same operation, arguments and kernel as mc_integrate, with these differences:
+ *   params        what mc_create would be given, validated the same way on every call (nothing is created; per-orbit
+ *                 parameter arrays must be valid for the duration of the launch); work is enqueued on
+ *                 params->cuda_stream of params->device.  chunk_steps and regroup are ignored (one chunk, caller's
+ *                 order: neither changes a result bit).  MC_TERM_RR is refused (MC_EINVAL): its extra outputs are
+ *                 only reachable through a handle
+ *   out_status    DEVICE int32[n_orbits] (mc_status) and
+ *   out_step      DEVICE int64[n_orbits] (completed steps): REQUIRED here, written by the kernel directly -- what
+ *                 mc_get_status would return
+ *   limit         n_orbits x (shadow_eps != 0 ? 2 : 1) <= MC_STATIC_MAX_TRAJECTORIES, else MC_ELIMIT and nothing
+ *                 is launched (mc_strerror(MC_ELIMIT) says so in words); larger batches need mc_integrate
+ * Results are those of mc_integrate on the same inputs, bit for bit.
+ *
+ * First call on a device: looks up the device address of the fixed array and the SM count (once per device, cached)
+ * and, like any first launch, makes the driver load the kernel.  Make that first call during start-up, before any
+ * stream capture begins.  Later calls do: argument checks, one 256-byte cudaMemsetAsync, one kernel launch.
+ *
+ * Sharing.  All calls on one device use the same array, and it keeps what the previous call left there; the entry
+ * point clears the part that must start at zero (the queue header) on the caller's stream.  Calls issued to the
+ * same stream therefore just queue up.  Two calls of one process whose kernels can overlap on the GPU (issued to
+ * different streams, from one host thread or several) would share one work queue: that is a data race with wrong
+ * results, and it is the caller's job to order them (one stream, or an event between them).  Separate processes
+ * each have their own copy of the array.
+ * Errors: MC_EINVAL, MC_ELIMIT (both before any CUDA call), MC_EARCH, MC_ECUDA. */
+#define MC_STATIC_MAX_TRAJECTORIES 32768
+int mc_integrate_static(const mc_params* params, const double* states, int64_t n_orbits, double step_h,
+                        int64_t n_steps, int32_t correction_mode, double shadow_eps, double* out_states,
+                        double* out_invariants, double* out_fli, int32_t* out_status, int64_t* out_step);
 
 /* Status of the orbits of the most recent mc_integrate on this handle, copied (stream-ordered) into
  * DEVICE arrays of the caller: out_status int32[n_orbits] (mc_status), out_step int64[n_orbits] =

@@ -13,11 +13,12 @@ from . import build as _build
 
 MC_TERM_1PN, MC_TERM_2PN, MC_TERM_SO, MC_TERM_S1S2, MC_TERM_QM, MC_TERM_RR = 1, 2, 4, 8, 16, 32
 TERMS_DEFAULT = MC_TERM_1PN | MC_TERM_2PN | MC_TERM_SO | MC_TERM_S1S2
-MC_OK, MC_EINVAL, MC_ECUDA, MC_EARCH, MC_ENOMEM = 0, -1, -2, -3, -4
+MC_OK, MC_EINVAL, MC_ECUDA, MC_EARCH, MC_ENOMEM, MC_ELIMIT = 0, -1, -2, -3, -4, -5
+MC_STATIC_MAX_TRAJECTORIES = 32768   # include/mc.h: the fixed scratch of mc_integrate_static
 MC_INTEG_RK4, MC_INTEG_RK5 = 0, 1
 
 # every symbol include/mc.h declares (tests/test_abi.py checks the header against this list)
-EXPORTS = ["mc_params_default", "mc_create", "mc_integrate", "mc_integrate_sampled", "mc_integrate_ex", "mc_carry_bytes", "mc_integrate_host", "mc_get_status", "mc_get_work", "mc_get_warp_work", "mc_get_dissipation", "mc_debug_check", "mc_eval",
+EXPORTS = ["mc_params_default", "mc_create", "mc_integrate", "mc_integrate_sampled", "mc_integrate_ex", "mc_carry_bytes", "mc_integrate_host", "mc_integrate_static", "mc_get_status", "mc_get_work", "mc_get_warp_work", "mc_get_dissipation", "mc_debug_check", "mc_eval",
            "mc_last_launch_info", "mc_fp64_peak", "mc_fp64_probe", "mc_flop_model", "mc_destroy", "mc_strerror"]
 
 
@@ -92,6 +93,7 @@ def load_library():
     lib.mc_integrate_ex.argtypes = [vp, vp, i64, dbl, i64, i32, dbl, vp, vp, vp, vp, i32]
     lib.mc_carry_bytes.argtypes = [i64, i32]
     lib.mc_integrate_host.argtypes = [vp, vp, i64, dbl, i64, i32, dbl, vp, vp, vp, vp, vp]
+    lib.mc_integrate_static.argtypes = [ctypes.POINTER(mc_params), vp, i64, dbl, i64, i32, dbl, vp, vp, vp, vp, vp]
     lib.mc_get_status.argtypes = [vp, vp, vp]
     lib.mc_get_work.argtypes = [vp, vp]
     lib.mc_get_dissipation.argtypes = [vp, vp]
@@ -318,6 +320,38 @@ class Integrator:
                                            fli.ctypes.data if fli is not None else None, status.ctypes.data,
                                            steps.ctypes.data))
         return IntegrateResult(out, inv, fli, status, steps)
+
+    def integrate_static(self, states, h, n_steps, correction_mode=3, shadow_eps=0.0, out=None) -> IntegrateResult:
+        """mc_integrate_static: the same integration for callers that must not allocate device memory (a process whose
+        own pool owns the whole GPU, a latency-bound loop that cannot afford cudaMalloc's stall, code running while a
+        stream is being captured).  The library keeps its bookkeeping in a fixed array inside libmc.so instead of
+        cudaMalloc'ed handle buffers, so the batch is limited to MC_STATIC_MAX_TRAJECTORIES trajectories (orbits, or
+        2 x orbits with a shadow; MCError with code MC_ELIMIT beyond that) and calls on different streams must not
+        overlap.  It takes this Integrator's parameters but not its handle.
+
+        `states` must already be a contiguous float64 device tensor (12, n) -- converting it would allocate.  `out`,
+        an IntegrateResult of preallocated device tensors (states, invariants or None, fli if shadow_eps != 0, status
+        int32, steps_done int64), receives the outputs; without it this wrapper allocates them through torch, which
+        is fine for a test and defeats the purpose in production."""
+        torch = self._torch
+        z = states
+        if not (isinstance(z, torch.Tensor) and z.device == self.device and z.dtype == torch.float64 and z.is_contiguous()
+                and z.dim() == 2 and z.shape[0] == 12):
+            raise ValueError("integrate_static needs a contiguous float64 (12, n) tensor on the integrator's device")
+        n = z.shape[1]
+        if self.n_params is not None and n > self.n_params:
+            raise ValueError("more orbits than per-orbit parameters")
+        if out is None:
+            out = IntegrateResult(torch.empty_like(z), torch.empty_like(z),
+                                  torch.empty(n, dtype=torch.float64, device=self.device) if shadow_eps != 0.0 else None,
+                                  torch.empty(n, dtype=torch.int32, device=self.device),
+                                  torch.empty(n, dtype=torch.int64, device=self.device))
+        _check(self._lib.mc_integrate_static(ctypes.byref(self.params), z.data_ptr(), n, float(h), int(n_steps),
+                                             int(correction_mode), float(shadow_eps), out.states.data_ptr(),
+                                             out.invariants.data_ptr() if out.invariants is not None else None,
+                                             out.fli.data_ptr() if out.fli is not None else None,
+                                             out.status.data_ptr(), out.steps_done.data_ptr()))
+        return out
 
     _WHAT = {"H": (0, 1), "rhs": (1, 12), "integrals": (2, 6), "rk4_step": (3, 12), "correct": (4, 12)}
 

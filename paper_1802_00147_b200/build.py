@@ -10,7 +10,7 @@ OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libmc.so")
 LIB_CHECKED = os.path.join(HERE, "libmc_checked.so")     # -DMC_CHECKED: index / pointer tests before every global access
 SOURCES = ["mc_api.cu", "mc_kernel_mode0.cu", "mc_kernel_mode1.cu", "mc_kernel_mode2.cu", "mc_kernel_mode3.cu",
-           "mc_flop_model.cpp"]       # .cpp: host-only C++ (the flop model), compiled by nvcc's host compiler
+           "mc_static.cu", "mc_flop_model.cpp"]       # .cpp: host-only C++ (the flop model), compiled by nvcc's host compiler
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

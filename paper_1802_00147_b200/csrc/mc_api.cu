@@ -49,6 +49,10 @@ struct DeviceBuf {
 
 }  // namespace
 
+namespace mc {
+int record_cuda_failure(cudaError_t e) { return cuda_fail(e); }
+}  // namespace mc
+
 struct mc_handle {
   mc_params P;
   McConsts uc;               // derived constants of the uniform parameter set
@@ -654,6 +658,7 @@ const char* mc_strerror(int code) {
     case MC_ECUDA: return g_cuda_msg;
     case MC_EARCH: return "device is not compute capability 10.x (library holds sm_100a code only)";
     case MC_ENOMEM: return "host allocation failed";
+    case MC_ELIMIT: return "batch too large for mc_integrate_static: its fixed device scratch holds at most 32768 trajectories (orbits, or 2 x orbits with a shadow); use mc_integrate";
     default: return "unknown mc_error";
   }
 }

@@ -15,4 +15,6 @@ LaunchFn launcher_mode0(int params, bool qm, int integrator, bool rr);
 LaunchFn launcher_mode1(int params, bool qm, int integrator, bool rr);
 LaunchFn launcher_mode2(int params, bool qm, int integrator, bool rr);
 LaunchFn launcher_mode3(int params, bool qm, int integrator, bool rr);
+// mc_api.cu: stores the text mc_strerror(MC_ECUDA) returns on this thread; returns MC_ECUDA (for mc_static.cu)
+int record_cuda_failure(cudaError_t e);
 }  // namespace mc

@@ -25,7 +25,7 @@ from paper_1802_00147_b200 import sharding, workloads  # noqa: E402
 
 METRIC = "orbit-RK4-steps/sec (with correction+FLI)"
 UNIT = "orbit-steps/s"
-# Algorithmic FP64 flops: NOT constants of this file.  They come from mc_flop_model (include/mc.h), which runs the
+# Algorithmic FP64 flops: NOT constants of this file.  They come from mc_flop_model (include/mc_bench.h, benchlib/), which runs the
 # kernels' own math templates with a counting scalar on the host (FMA = 2, add/mul = 1, rsqrt/reciprocal/division/
 # sqrt = 1; the Newton refinements around the hardware seeds are not algorithmic work) -- see algorithmic_flop()
 # below and tests/test_flop_model.py.  The number of Gauss-Newton steps of mode 3 is data dependent (epsilon-
@@ -59,6 +59,11 @@ def parse_args():
     ap.add_argument("--regroup", action="store_true",
                     help="mc_params.regroup: integrate the orbits in energy order (index mapping only; profiles/ tables only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1, config2 only: weak (default, the driver's contract) = 314 N rows, 314 per GPU; strong = the SAME "
+                         "314 x 314 scan dealt row by row over the N GPUs (SURVEY 8e: n/G orbits per GPU)")
+    ap.add_argument("--tabulate", default=None, metavar="FILE.jsonl",
+                    help="no GPU work: print a markdown table of the bench lines in FILE.jsonl (profiles/ tables are made this way)")
     return ap.parse_args()
 
 
@@ -116,8 +121,8 @@ def algorithmic_flop(w, mode, integrator, steps_done, gn_steps):
     orbit summed over orbit and shadow (`gn_steps`, mc_get_work).  A trajectory-step = base integrator step +
     the per-step part of the correction + status test; with a shadow every accepted orbit-step is two
     trajectory-steps and every renorm_interval-th step one renormalisation."""
-    from paper_1802_00147_b200 import binding
-    m = binding.flop_model(w.terms, mode, integrator)
+    import benchlib
+    m = benchlib.flop_model(w.terms, mode, integrator)
     traj = 2 if w.shadow_eps != 0.0 else 1
     steps_done = np.asarray(steps_done, dtype=np.int64)
     per_traj_step = m["base_step"]["flop"] + m["correct_fixed"]["flop"] + m["status"]["flop"]
@@ -135,7 +140,7 @@ def executed_from_sass(w, rk5, warp_work, per_launch_s, num_sms, sm_mhz, value):
     the library's own object file) times the warp-level work counters of the launch (mc_get_warp_work), and the time
     the FP64 pipe needs for it under the measured operand-bandwidth rule (3 cycles for an FMA with three distinct
     register operands, 2 otherwise; mc_fp64_probe).  None for kernels the SASS reader does not handle."""
-    from paper_1802_00147_b200 import sass_mix
+    from benchlib import sass_mix
     if rk5 or w.correction_mode != 3 or (w.terms & 32) or not warp_work["warp_steps"]:
         return None
     params = 0 if w.uniform else (2 if (w.terms & 16 and len(set(w.beta)) == 1 and len(set(w.chi1)) == 1 and len(set(w.chi2)) == 1) else
@@ -148,7 +153,7 @@ def executed_from_sass(w, rk5, warp_work, per_launch_s, num_sms, sm_mhz, value):
     flop = per["flop"] * 32.0 * warp_work["warp_steps"]              # every lane slot of every executed warp instruction
     cycles = per["cycles"] * warp_work["warp_steps"] / (4.0 * num_sms)   # per sub-partition, perfectly balanced
     model_s = cycles / (sm_mhz * 1e6)
-    return {"source": "SASS mix of the built library (paper_1802_00147_b200/sass_mix.py) x mc_get_warp_work",
+    return {"source": "SASS mix of the built library (benchlib/sass_mix.py) x mc_get_warp_work",
             "gn_passes_per_warp_step": g, "fp64_instr_per_warp_step": per["fp64"], "dfma_3_register_per_warp_step": per["dfma_3reg"],
             "dfma_share_of_fp64_instr": per["DFMA"] / per["fp64"], "executed_flop_per_launch": flop,
             "executed_tflops": flop / per_launch_s / 1e12,
@@ -163,7 +168,8 @@ def global_workload(args, world):
     name, _, opt = args.workload.partition(":")
     kw = {} if args.n_steps is None else {"n_steps": args.n_steps}
     if name == "config2":
-        w = workloads.config2(n_r=args.grid * world, n_theta=args.grid, **kw)
+        strong = getattr(args, "scaling", "weak") == "strong"
+        w = workloads.config2(n_r=args.grid * (1 if strong else world), n_theta=args.grid, **kw)
         if opt == "rr":                             # the same scan with the 2.5PN radiation reaction (MC_TERM_RR)
             w.terms |= 32
         return w
@@ -188,13 +194,16 @@ def global_workload(args, world):
 def rank_shard(w, args, rank, world):
     if args.workload.partition(":")[0] != "config2":
         return w
+    if getattr(args, "scaling", "weak") == "strong":
+        return sharding.strong_shard(w, args.grid, args.grid, rank, world)
     return sharding.rank_shard(w, args.grid, args.grid, rank, world)
 
 
 def describe(w, args):
     integ = "RK5 (Butcher six-stage)" if args.integrator == "rk5" else "RK4"
     if w.name.startswith("config2"):
-        return (f"config2: {args.grid}x{args.grid} orbit scan per GPU (r0 in [10,60] x theta in [0,pi]), equal mass, chi=1, "
+        per = "in total, rows dealt over the GPUs" if getattr(args, "scaling", "weak") == "strong" else "per GPU"
+        return (f"config2: {args.grid}x{args.grid} orbit scan {per} (r0 in [10,60] x theta in [0,pi]), equal mass, chi=1, "
                 f"N+1PN+2PN+SO+SS{'+2.5PN radiation reaction' if w.terms & 32 else ''}, {integ} h=1, {w.n_steps} steps, shadow 1e-8 renormalised every 100 steps + FLI, "
                 + ("six-integral correction (mode 3, Gauss-Newton terminated at eps=1e-10, cap 4)" if w.correction_mode == 3
                    else f"correction mode {w.correction_mode}"))
@@ -287,8 +296,9 @@ def run_mc(args):
     z_pin = torch.as_tensor(w.states).pin_memory()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
 
-    peak_tf, peak_clock = binding.fp64_peak(local, 200.0) if rank == 0 else (None, None)
-    probe = binding.fp64_probe(local, 50.0) if rank == 0 else None      # operand-bandwidth rule of the FP64 pipe, measured here
+    import benchlib
+    peak_tf, peak_clock = benchlib.fp64_peak(local, 200.0) if rank == 0 else (None, None)
+    probe = benchlib.fp64_probe(local, 50.0) if rank == 0 else None      # operand-bandwidth rule of the FP64 pipe, measured here
     if w.uniform:
         par = dict(beta=float(w.beta[0]), chi1=float(w.chi1[0]), chi2=float(w.chi2[0]), kq1=float(w.kq1[0]), kq2=float(w.kq2[0]))
     else:
@@ -350,6 +360,7 @@ def run_mc(args):
     steps_done = float(steps_done_per_orbit.sum())            # accepted orbit-steps of one launch (this rank)
     gn_steps = float(gn_per_orbit.sum())                      # Gauss-Newton steps of one launch, orbit + shadow
     steps_done_job = sharding.sum_over_ranks(steps_done, dev)
+    scheduled_job = sharding.sum_over_ranks(orbit_steps_rank, dev)
     # orbit-steps actually integrated (dropped cells stop counting when they freeze), whole job
     value = steps_done_job * args.steps / (dev_ms_max * 1e-3)
     e2e_value = steps_done_job * args.steps / e2e_s_max
@@ -398,13 +409,13 @@ def run_mc(args):
                 "blocks_per_sm": info["blocks_per_sm"], "grid": info["grid"], "block": info["block"]}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dev_ms_max / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "scaling": args.scaling if w.name.startswith("config2") else "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": describe(w, args),
                        "orbits_per_gpu": n, "rk4_steps": w.n_steps, "sample_interval": args.sample_interval,
                        "sample_bytes_per_launch": (w.n_steps // args.sample_interval) * 96 * n if args.sample_interval else 0,
                        "orbit_steps_counted": "accepted steps (sum of steps_done); scheduled = orbits x rk4_steps = %d" % int(orbit_steps_rank * world), "l2": "flushed (256 MiB write) between timed iterations",
                        "regroup": bool(args.regroup),
-                       "parallelism": f"orbit-sharded x{world} (grid rows round-robin over ranks), no collective"},
+                       "parallelism": f"orbit-sharded x{world} (grid rows round-robin over ranks; {args.scaling} scaling), no collective"},
             "clocks": clocks, "wall_s_timed_region": t_wall,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
             "gpu_launches": launches, "roofline": roofline,
@@ -418,8 +429,38 @@ def run_mc(args):
         dist.destroy_process_group()
 
 
+TABLE_COLUMNS = [("workload", lambda l: l["config"]["workload"].split(": ")[0] + (" regroup" if l["config"].get("regroup") else "")),
+                 ("kernel", lambda l: l["roofline"]["kernel"].replace("mc::integrate_kernel", "")),
+                 ("orbits per GPU", lambda l: l["config"]["orbits_per_gpu"]),
+                 ("steps", lambda l: l["config"]["rk4_steps"]),
+                 ("orbit-steps/s", lambda l: "%.3e" % l["value"]),
+                 ("ms per launch", lambda l: "%.1f" % l["ms_per_step"]),
+                 ("TFLOP/s", lambda l: "%.2f" % l["roofline"]["achieved"]),
+                 ("frac", lambda l: "%.3f" % l["roofline"]["frac"]),
+                 ("regs", lambda l: l["roofline"]["regs_per_thread"]),
+                 ("spill B", lambda l: l["roofline"]["spill_bytes"]),
+                 ("blocks/SM", lambda l: l["roofline"]["blocks_per_sm"]),
+                 ("grid", lambda l: l["roofline"]["grid"]),
+                 ("GN steps per lane-step", lambda l: "%.3f" % l["roofline"]["gn_steps_per_trajectory_step"]),
+                 ("regular / chaotic / dropped", lambda l: "%d / %d / %d" % (l["outcome"]["regular"], l["outcome"]["chaotic"], l["outcome"]["dropped"])),
+                 ("SM MHz (median / max)", lambda l: "%s / %s" % (l["clocks"]["sm_mhz"], l["clocks"]["sm_max_mhz"])),
+                 ("throttle reasons", lambda l: ", ".join(l["clocks"]["reasons"]) or "none"),
+                 ("power W max", lambda l: l["clocks"]["power_w_max"])]
+
+
+def tabulate(path):
+    """Markdown table of the bench lines in a .jsonl file: one row per line, the clock record of the run beside its number."""
+    lines = [json.loads(t) for t in open(path) if t.strip().startswith("{")]
+    print("| " + " | ".join(name for name, _ in TABLE_COLUMNS) + " |")
+    print("|" + "---|" * len(TABLE_COLUMNS))
+    for l in lines:
+        print("| " + " | ".join(str(fn(l)) for _, fn in TABLE_COLUMNS) + " |")
+
+
 def main():
     args = parse_args()
+    if args.tabulate:
+        return tabulate(args.tabulate)
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -1,10 +1,10 @@
-// mc_flop_model.cpp -- mc_flop_model (include/mc.h): the algorithmic operation counts of the kernels'
+// mc_flop_model.cpp -- mc_flop_model (include/mc_bench.h; built into benchlib/libmc_bench.so): the algorithmic operation counts of the kernels'
 // own formulation, obtained by running the kernels' math templates (mc_math.cuh, mc_correct.cuh) once on the
 // host with the counting scalar mc::Cnt.  Plain C++ (no CUDA): works on a box without a GPU.
 #include <cstring>
 
-#include "../../include/mc.h"
-#include "mc_count.h"
+#include "../include/mc_bench.h"
+#include "mc_count.h"      // -I paper_1802_00147_b200/csrc: the kernels' own math templates
 #include "mc_correct.cuh"
 
 namespace {

@@ -1,6 +1,6 @@
 """Executed instruction mix of the hot kernel's step loop, read from the SASS of the library that was just built.
 
-    python -m paper_1802_00147_b200.sass_mix            # table for integrate_kernel<uniform, QM off, mode 3, RK4>
+    python -m benchlib.sass_mix            # table for integrate_kernel<uniform, QM off, mode 3, RK4>
 
 Why: bench.py reports ALGORITHMIC flop (mc_flop_model).  The flop the device really executes are a little higher
 (Newton refinements around the MUFU seeds, lanes idling through a neighbour's second Gauss-Newton step), and the
@@ -19,7 +19,7 @@ import os
 import re
 import subprocess
 
-from . import build as _build
+from paper_1802_00147_b200 import build as _build
 
 CYC_3RF, CYC_REUSE, CYC_PLAIN = 3.03, 2.19, 2.03      # cycles per warp instruction per sub-partition (mc_fp64_probe, B200)
 _PAT = re.compile(r"/\*([0-9a-f]{4,})\*/\s+(@!?U?P\w+\s+)?([A-Z0-9_.]+)\s*([^;]*);")

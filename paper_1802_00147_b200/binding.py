@@ -19,7 +19,7 @@ MC_INTEG_RK4, MC_INTEG_RK5 = 0, 1
 
 # every symbol include/mc.h declares (tests/test_abi.py checks the header against this list)
 EXPORTS = ["mc_params_default", "mc_create", "mc_integrate", "mc_integrate_sampled", "mc_integrate_ex", "mc_carry_bytes", "mc_integrate_host", "mc_integrate_static", "mc_get_status", "mc_get_work", "mc_get_warp_work", "mc_get_dissipation", "mc_debug_check", "mc_eval",
-           "mc_last_launch_info", "mc_fp64_peak", "mc_fp64_probe", "mc_flop_model", "mc_destroy", "mc_strerror"]
+           "mc_last_launch_info", "mc_destroy", "mc_strerror"]
 
 
 class MCLibraryError(RuntimeError):
@@ -48,14 +48,6 @@ class mc_launch_info(ctypes.Structure):
                 ("local_bytes", ctypes.c_int32), ("blocks_per_sm", ctypes.c_int32), ("num_sms", ctypes.c_int32),
                 ("smem_bytes", ctypes.c_int32), ("variant", ctypes.c_int32), ("trajectories", ctypes.c_int64),
                 ("chunk_steps", ctypes.c_int32), ("n_chunks", ctypes.c_int32)]
-
-
-class mc_op_counts(ctypes.Structure):
-    _fields_ = [("fma", ctypes.c_int64), ("mul", ctypes.c_int64), ("add", ctypes.c_int64), ("special", ctypes.c_int64)]
-
-
-class mc_flop_model_t(ctypes.Structure):
-    _fields_ = [(k, mc_op_counts) for k in ("rhs", "base_step", "correct_fixed", "gn_step", "status", "references", "renorm")]
 
 
 _lib = None
@@ -101,9 +93,6 @@ def load_library():
     lib.mc_debug_check.argtypes = [vp, ctypes.POINTER(ctypes.c_int64)]
     lib.mc_eval.argtypes = [vp, i32, vp, i64, dbl, i32, vp, vp]
     lib.mc_last_launch_info.argtypes = [vp, ctypes.POINTER(mc_launch_info)]
-    lib.mc_fp64_peak.argtypes = [i32, dbl, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
-    lib.mc_fp64_probe.argtypes = [i32, dbl, i32, ctypes.POINTER(dbl), ctypes.POINTER(dbl)]
-    lib.mc_flop_model.argtypes = [ctypes.c_uint32, i32, i32, i32, ctypes.POINTER(mc_flop_model_t)]
     lib.mc_destroy.argtypes = [vp]
     lib.mc_strerror.argtypes = [ctypes.c_int]
     lib.mc_strerror.restype = ctypes.c_char_p
@@ -124,39 +113,6 @@ def params_default() -> mc_params:
     p = mc_params()
     _check(load_library().mc_params_default(ctypes.byref(p)))
     return p
-
-
-def fp64_peak(device: int = 0, millis: float = 200.0):
-    """(TFLOP/s, implied SM clock in MHz) of the DFMA probe in libmc."""
-    t, c = ctypes.c_double(), ctypes.c_double()
-    _check(load_library().mc_fp64_peak(device, millis, ctypes.byref(t), ctypes.byref(c)))
-    return t.value, c.value
-
-
-FP64_PROBE_KINDS = {0: "fma(y,z,x): 3 registers", 1: "fma(y,s,x): 2 registers + reused", 2: "fma(y,c[],x): 2 registers + constant",
-                    3: "x*y: DMUL"}
-
-
-def fp64_probe(device: int = 0, millis: float = 100.0) -> dict:
-    """mc_fp64_probe for every kind: {kind name: (cycles per warp instruction per sub-partition, TFLOP/s)}."""
-    out = {}
-    for kind, name in FP64_PROBE_KINDS.items():
-        c, t = ctypes.c_double(), ctypes.c_double()
-        _check(load_library().mc_fp64_probe(device, millis, kind, ctypes.byref(c), ctypes.byref(t)))
-        out[name] = (c.value, t.value)
-    return out
-
-
-def flop_model(terms=TERMS_DEFAULT, correction_mode=3, integrator=0, newton_iters=4) -> dict:
-    """mc_flop_model: operation counts of the kernels' own formulation, per trajectory (host-only, no GPU needed).
-    Returns {part: {"fma", "mul", "add", "special", "flop"}} with flop = 2 fma + mul + add + special."""
-    m = mc_flop_model_t()
-    _check(load_library().mc_flop_model(int(terms), int(correction_mode), int(integrator), int(newton_iters), ctypes.byref(m)))
-    out = {}
-    for part, _ in mc_flop_model_t._fields_:
-        c = getattr(m, part)
-        out[part] = dict(fma=c.fma, mul=c.mul, add=c.add, special=c.special, flop=2 * c.fma + c.mul + c.add + c.special)
-    return out
 
 
 @dataclass
@@ -194,6 +150,9 @@ class Integrator:
             """The scalar all orbits share, or None if the parameter really varies."""
             if not hasattr(v, "__len__"):
                 return float(v)
+            if isinstance(v, torch.Tensor):          # device tensors stay where they are: tested with torch, no host copy of the array
+                t = v.detach().reshape(-1)
+                return float(t[0]) if t.numel() and bool((t == t[0]).all()) else None
             import numpy as np
             a = np.asarray(v, dtype=np.float64)
             return float(a.flat[0]) if a.size and (a == a.flat[0]).all() else None

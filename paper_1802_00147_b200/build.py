@@ -10,7 +10,7 @@ OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libmc.so")
 LIB_CHECKED = os.path.join(HERE, "libmc_checked.so")     # -DMC_CHECKED: index / pointer tests before every global access
 SOURCES = ["mc_api.cu", "mc_kernel_mode0.cu", "mc_kernel_mode1.cu", "mc_kernel_mode2.cu", "mc_kernel_mode3.cu",
-           "mc_static.cu", "mc_flop_model.cpp"]       # .cpp: host-only C++ (the flop model), compiled by nvcc's host compiler
+           "mc_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
@@ -18,7 +18,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3",
 def _deps():
     out = [os.path.join(HERE, "..", "include", "mc.h")]
     for f in os.listdir(CSRC):
-        if f.endswith((".cu", ".cuh", ".h", ".cpp")):
+        if f.endswith((".cu", ".cuh", ".h")):
             out.append(os.path.join(CSRC, f))
     return out
 
@@ -97,11 +97,6 @@ def _build_locked(obj_dir: str, verbose: bool, checked: bool) -> str:
     os.replace(lib + ".tmp", lib)
     if checked:
         return lib
-    try:                                    # SASS instruction mix of the hot loop, for bench.py's `roofline.executed`
-        from . import sass_mix
-        sass_mix.write_json()
-    except Exception as e:                  # cuobjdump missing: bench.py reports executed = null
-        print(f"sass_mix skipped: {e}")
     return LIB
 
 

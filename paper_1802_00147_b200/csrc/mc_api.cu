@@ -1,5 +1,5 @@
 // mc_api.cu -- the C ABI of include/mc.h: handle, validation, launches, host-buffer variant,
-// evaluation entry point for the parity tests, FP64 peak probe.
+// evaluation entry point for the parity tests.  (The bench's instruments live in benchlib/, not here.)
 #include <cuda_runtime.h>
 #include <cub/device/device_radix_sort.cuh>
 
@@ -155,63 +155,6 @@ energy_key_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ m
   }
 }
 
-// ---- DFMA throughput probe -------------------------------------------------------------------------
-// 16 independent FMA chains per thread, 256 threads per block, 8 blocks per SM resident.
-__global__ void __launch_bounds__(256)
-dfma_peak_kernel(double* sink, int iters, double a, double b) {
-  double x[16];
-#pragma unroll
-  for (int j = 0; j < 16; ++j) x[j] = 1.0 + 1e-9 * (threadIdx.x + j);
-#pragma unroll 1
-  for (int i = 0; i < iters; ++i) {
-#pragma unroll
-    for (int rep = 0; rep < 8; ++rep) {
-#pragma unroll
-      for (int j = 0; j < 16; ++j) x[j] = fma(x[j], a, b);
-    }
-  }
-  double s = 0.0;
-#pragma unroll
-  for (int j = 0; j < 16; ++j) s += x[j];
-  if (s == 123.456) sink[0] = s;   // never true: keeps the chains alive
-}
-
-// Operand-bandwidth probe (mc_fp64_probe): 8 independent accumulators per thread, x_j <- fma(y_j, *, x_j).
-//   KIND 0: fma(y_j, z_j, x_j) -- three distinct vector registers per instruction
-//   KIND 1: fma(y_j, s,   x_j) -- two + one register shared by consecutive instructions (operand reuse cache)
-//   KIND 2: fma(y_j, c[], x_j) -- two registers + a constant-bank operand
-//   KIND 3: x_j * y_j          -- DMUL, two registers
-__constant__ double g_probe_const[2];
-template <int KIND>
-__global__ void __launch_bounds__(128)
-dfma_operand_probe_kernel(double* sink, int iters, double a, double b) {
-  double x[8], y[8], z[8];
-#pragma unroll
-  for (int j = 0; j < 8; ++j) {
-    x[j] = 1.0 + 1e-9 * (threadIdx.x + j);
-    y[j] = 0.9999999 + 1e-12 * (threadIdx.x + 3 * j) * a;
-    z[j] = 1e-9 * (1 + j) * b + 1e-15 * threadIdx.x;
-  }
-  const double s = a + 1e-15 * threadIdx.x;
-#pragma unroll 1
-  for (int i = 0; i < iters; ++i) {
-#pragma unroll
-    for (int rep = 0; rep < 8; ++rep) {
-#pragma unroll
-      for (int j = 0; j < 8; ++j) {
-        if (KIND == 0) x[j] = fma(y[j], z[j], x[j]);
-        else if (KIND == 1) x[j] = fma(y[j], s, x[j]);
-        else if (KIND == 2) x[j] = fma(y[j], g_probe_const[1], x[j]);
-        else x[j] = x[j] * y[j];
-      }
-    }
-  }
-  double t = 0.0;
-#pragma unroll
-  for (int j = 0; j < 8; ++j) t += x[j] + y[j] + z[j];
-  if (t == 123.456) sink[0] = t + s;   // never true: keeps the chains alive
-}
-
 void fill_args(const mc_handle* h, mc::IntegrateArgs& A) {
   memset(&A, 0, sizeof(A));
   A.beta = h->P.d_beta; A.chi1 = h->P.d_chi1; A.chi2 = h->P.d_chi2; A.kq1 = h->P.d_kq1; A.kq2 = h->P.d_kq2;
@@ -333,16 +276,29 @@ static int integrate_impl(mc_handle* h, const double* states, int64_t n_orbits, 
   const bool shadow = shadow_eps != 0.0;
   if (n_orbits > 0 && ((!states && !resume) || !out_states || (shadow && !out_fli))) return MC_EINVAL;
   if (n_orbits > (int64_t)1 << 40) return MC_EINVAL;
+  // everything that can be refused is refused before the handle's record of the last launch (last_n) is touched:
+  // after a failed call mc_get_status / mc_get_work still describe the last launch that did run
+  const bool qm = (h->P.terms & MC_TERM_QM) != 0;
+  const bool rr = (h->P.terms & MC_TERM_RR) != 0;
+  mc::LaunchFn fn = nullptr;
+  switch (correction_mode) {
+    case 0: fn = mc::launcher_mode0(h->P.per_orbit, qm, h->P.integrator, rr); break;
+    case 1: fn = mc::launcher_mode1(h->P.per_orbit, qm, h->P.integrator, rr); break;
+    case 2: fn = mc::launcher_mode2(h->P.per_orbit, qm, h->P.integrator, rr); break;
+    default: fn = mc::launcher_mode3(h->P.per_orbit, qm, h->P.integrator, rr); break;
+  }
+  if (!fn) return MC_EINVAL;   // per_orbit = 1 with RK5 and MC_TERM_RR: not built (register budget; include/mc.h)
+  const int64_t traj = n_orbits * (shadow ? 2 : 1);
+  if ((traj + 31) / 32 > 0x3fffffffLL) return MC_EINVAL;
   MC_CUDA(cudaSetDevice(h->P.device));
-  h->last_n = n_orbits;
-  if (n_orbits == 0) return MC_OK;
+  if (n_orbits == 0) { h->last_n = 0; return MC_OK; }
+  h->last_n = 0;               // until the launch below has been enqueued the status buffers describe nothing
   int rc = h->status.reserve(sizeof(int32_t) * (size_t)n_orbits);
   if (rc) return rc;
   rc = h->step.reserve(sizeof(int64_t) * (size_t)n_orbits);
   if (rc) return rc;
   rc = h->gn.reserve(sizeof(int64_t) * (size_t)n_orbits);
   if (rc) return rc;
-  const bool rr = (h->P.terms & MC_TERM_RR) != 0;
   if (rr && (rc = h->diss.reserve(sizeof(double) * 4 * (size_t)n_orbits))) return rc;
 
   mc::IntegrateArgs A;
@@ -354,18 +310,7 @@ static int integrate_impl(mc_handle* h, const double* states, int64_t n_orbits, 
   A.samples = sample_interval > 0 ? out_samples : nullptr;
   A.sample_interval = sample_interval > 0 ? (int32_t)sample_interval : 1;
 
-  const bool qm = (h->P.terms & MC_TERM_QM) != 0;
-  mc::LaunchFn fn = nullptr;
-  switch (correction_mode) {
-    case 0: fn = mc::launcher_mode0(h->P.per_orbit, qm, h->P.integrator, rr); break;
-    case 1: fn = mc::launcher_mode1(h->P.per_orbit, qm, h->P.integrator, rr); break;
-    case 2: fn = mc::launcher_mode2(h->P.per_orbit, qm, h->P.integrator, rr); break;
-    default: fn = mc::launcher_mode3(h->P.per_orbit, qm, h->P.integrator, rr); break;
-  }
-  if (!fn) return MC_EINVAL;   // per_orbit = 1 with RK5 and MC_TERM_RR: not built (register budget; include/mc.h)
-  const int64_t traj = n_orbits * (shadow ? 2 : 1);
   A.n_units = (traj + 31) / 32;
-  if (A.n_units > 0x3fffffffLL) return MC_EINVAL;
   A.chunk_len = 1; A.n_chunks = 1; A.n_items = A.n_units;
   mc::KernelInfo ki;
   MC_CUDA(fn(h->uc, A, h->num_sms, false, h->stream, &ki));                  // occupancy / register query
@@ -382,6 +327,10 @@ static int integrate_impl(mc_handle* h, const double* states, int64_t n_orbits, 
     if (shadow) chunk = ((chunk + ri - 1) / ri) * ri;
   }
   if (chunk > 0x7fffffffLL) chunk = 0x7fffffffLL;
+  // the kernel counts the Gauss-Newton steps and warp passes of ONE work item in 32 bits (at most newton_iters per
+  // step) and adds them to 64-bit totals at chunk boundaries: keep chunk_len * newton_iters below 2^32
+  const int64_t counter_cap = 0xffffffffLL / h->P.newton_iters;
+  if (chunk > counter_cap) chunk = counter_cap;
   int64_t n_chunks = n_steps > 0 ? (n_steps + chunk - 1) / chunk : 1;
   if (n_chunks > 0x7fffffffLL) return MC_EINVAL;
   A.chunk_len = (int32_t)chunk;
@@ -448,6 +397,7 @@ static int integrate_impl(mc_handle* h, const double* states, int64_t n_orbits, 
   const int kparams = (h->P.per_orbit == 2 && !qm) ? 0 : h->P.per_orbit;   // kappa is unused without the QM term
   h->info.variant = (kparams == 1 ? 1 : 0) | (qm ? 2 : 0) | (kparams == 2 ? 4 : 0) | (rr ? 8 : 0) | (correction_mode << 4) | (h->P.integrator << 8) | (A.perm ? 1024 : 0);
   h->info.trajectories = traj;
+  h->last_n = n_orbits;
   return MC_OK;
 }
 
@@ -558,85 +508,6 @@ int mc_eval(mc_handle* h, int32_t what, const double* states, int64_t n, double 
 int mc_last_launch_info(mc_handle* h, mc_launch_info* out) {
   if (!h || !out) return MC_EINVAL;
   *out = h->info;
-  return MC_OK;
-}
-
-int mc_fp64_peak(int32_t device, double millis, double* out_tflops, double* out_sm_clock_mhz) {
-  if (!out_tflops || !(millis > 0.0)) return MC_EINVAL;
-  MC_CUDA(cudaSetDevice(device));
-  cudaDeviceProp prop;
-  MC_CUDA(cudaGetDeviceProperties(&prop, device));
-  double* sink = nullptr;
-  MC_CUDA(cudaMalloc(&sink, sizeof(double)));
-  cudaEvent_t e0, e1;
-  MC_CUDA(cudaEventCreate(&e0));
-  MC_CUDA(cudaEventCreate(&e1));
-  const int grid = prop.multiProcessorCount * 8, block = 256;
-  int iters = 2000;
-  double best = 0.0;
-  float ms = 0.f;
-  for (int pass = 0; pass < 6; ++pass) {
-    MC_CUDA(cudaEventRecord(e0, 0));
-    dfma_peak_kernel<<<grid, block>>>(sink, iters, 0.999999999, 1e-9);
-    MC_CUDA(cudaEventRecord(e1, 0));
-    MC_CUDA(cudaEventSynchronize(e1));
-    MC_CUDA(cudaEventElapsedTime(&ms, e0, e1));
-    const double flops = 2.0 * 16.0 * 8.0 * (double)iters * (double)grid * block;
-    const double tf = flops / (ms * 1e-3) / 1e12;
-    if (pass >= 2 && tf > best) best = tf;               // passes 0-1 size the run and warm the clocks
-    if (pass < 2 && ms > 0.f) iters = (int)fmin(2.0e6, fmax(100.0, iters * millis / ms));
-  }
-  *out_tflops = best;
-  if (out_sm_clock_mhz) {
-    // cycles per second implied by one DFMA per lane per clock on 64 lanes per SM
-    *out_sm_clock_mhz = best * 1e12 / (2.0 * 64.0 * prop.multiProcessorCount) / 1e6;
-  }
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  cudaFree(sink);
-  return MC_OK;
-}
-
-int mc_fp64_probe(int32_t device, double millis, int32_t kind, double* out_cycles_per_warp_instr, double* out_tflops) {
-  if (!out_cycles_per_warp_instr || !(millis > 0.0) || kind < 0 || kind > 3) return MC_EINVAL;
-  MC_CUDA(cudaSetDevice(device));
-  cudaDeviceProp prop;
-  MC_CUDA(cudaGetDeviceProperties(&prop, device));
-  const double hc[2] = {0.0, 0.999999999};
-  MC_CUDA(cudaMemcpyToSymbol(g_probe_const, hc, sizeof(hc)));
-  double* sink = nullptr;
-  MC_CUDA(cudaMalloc(&sink, sizeof(double)));
-  cudaEvent_t e0, e1;
-  MC_CUDA(cudaEventCreate(&e0));
-  MC_CUDA(cudaEventCreate(&e1));
-  const int warps_per_smsp = 4, block = 128, grid = prop.multiProcessorCount * warps_per_smsp;   // one warp per sub-partition per block
-  int iters = 2000;
-  float ms = 0.f, best = 1e30f;
-  for (int pass = 0; pass < 6; ++pass) {
-    MC_CUDA(cudaEventRecord(e0, 0));
-    switch (kind) {
-      case 0: dfma_operand_probe_kernel<0><<<grid, block>>>(sink, iters, 0.999999999, 1e-9); break;
-      case 1: dfma_operand_probe_kernel<1><<<grid, block>>>(sink, iters, 0.999999999, 1e-9); break;
-      case 2: dfma_operand_probe_kernel<2><<<grid, block>>>(sink, iters, 0.999999999, 1e-9); break;
-      default: dfma_operand_probe_kernel<3><<<grid, block>>>(sink, iters, 0.999999999, 1e-9); break;
-    }
-    MC_CUDA(cudaEventRecord(e1, 0));
-    MC_CUDA(cudaEventSynchronize(e1));
-    MC_CUDA(cudaEventElapsedTime(&ms, e0, e1));
-    if (pass >= 2 && ms < best) best = ms;
-    if (pass < 2 && ms > 0.f) iters = (int)fmin(2.0e6, fmax(100.0, iters * millis / ms));
-  }
-  // warp instructions per sub-partition = iters * 64 * warps_per_smsp; cycles at the device's maximum SM clock
-  const double inst = (double)iters * 64.0 * warps_per_smsp;
-  const double clk = prop.clockRate * 1e3;
-  *out_cycles_per_warp_instr = best * 1e-3 * clk / inst;
-  if (out_tflops) {
-    const double flop_per_inst = kind == 3 ? 1.0 : 2.0;
-    *out_tflops = flop_per_inst * 32.0 * inst * 4.0 * prop.multiProcessorCount / (best * 1e-3) / 1e12;
-  }
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  cudaFree(sink);
   return MC_OK;
 }
 

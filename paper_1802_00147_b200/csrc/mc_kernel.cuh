@@ -191,8 +191,10 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
           else if (now - t0 > A.wait_budget_ns) __trap();         // fail loudly instead of hanging
         }
       }
+      // acquire, mirroring the publish side below: the lane that observed the flag issues the fence, the barrier then
+      // orders every lane's ld.cg after it (a resumed chunk 0 has no flag to observe: the previous launch has ended)
+      if (lane == 0) __threadfence();
       __syncwarp();
-      __threadfence();
       MC_CHK(A.carry_d != nullptr && A.carry_i != nullptr && A.carry_g != nullptr && A.done != nullptr);
 #pragma unroll
       for (int i = 0; i < 12; ++i) y[i] = __ldcg(A.carry_d + (int64_t)i * tp + t);   // L2 only: L1 may be stale

@@ -29,6 +29,17 @@ def rank_shard(w: Workload, n_rows_per_rank: int, n_cols: int, rank: int, world_
     return w.subset(rank_orbits(n_rows_per_rank, n_cols, rank, world_size))
 
 
+def strong_orbits(n_rows: int, n_cols: int, rank: int, world_size: int) -> np.ndarray:
+    """Strong scaling: the SAME (n_rows x n_cols) grid dealt over the ranks, row i to rank i mod N.  Ranks hold
+    ceil(n_rows / N) or floor(n_rows / N) rows (314 rows over 8 ranks: 40, 40, 39, ...: 12 560 or 12 246 orbits)."""
+    rows = np.arange(rank, n_rows, world_size)
+    return (rows[:, None] * n_cols + np.arange(n_cols)[None, :]).ravel()
+
+
+def strong_shard(w: Workload, n_rows: int, n_cols: int, rank: int, world_size: int) -> Workload:
+    return w.subset(strong_orbits(n_rows, n_cols, rank, world_size))
+
+
 def scatter_back(parts, n_rows_per_rank: int, n_cols: int, world_size: int) -> np.ndarray:
     """Inverse of the split for an output array: parts[r] has the rank-local orbit axis last; returns the global
     array (outputs of different ranks are disjoint slices, so this is a permutation, not a reduction)."""

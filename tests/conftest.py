@@ -32,3 +32,14 @@ def random_states(n, seed, r_scale=(8.0, 40.0), p_scale=(0.1, 0.35)):
 @pytest.fixture
 def rand_states():
     return random_states
+
+
+def config3_sample():
+    """The cells of BASELINE config 3 that the full-length class tests recompute with the oracle: 400 drawn uniformly from
+    the 314 x 314 grid (north_star's bar is on grid cells) + 100 more from the strong-field rows r0 < 18, where every
+    chaotic and dropped cell lives.  Returns (global cell indices, mask of the uniform part)."""
+    rng = np.random.default_rng(8)
+    uni = rng.choice(314 * 314, 400, replace=False)
+    strong = np.setdiff1d(rng.choice(314 * 50, 110, replace=False), uni)[:100]
+    idx = np.concatenate([uni, strong])
+    return idx, np.arange(idx.size) < uni.size

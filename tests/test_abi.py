@@ -26,10 +26,27 @@ def test_library_exports_every_declared_symbol():
         assert hasattr(lib, n), n
 
 
+def test_bench_instruments_are_a_library_of_their_own():
+    """include/mc_bench.h (FP64 probes, flop model) is served by benchlib/libmc_bench.so; libmc.so, the product, exports
+    none of it, and the product package does not import the bench package."""
+    import benchlib
+    src = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "mc_bench.h")).read(), flags=re.S)
+    names = sorted(set(re.findall(r"\b(mc_[a-z0-9_]+)\s*\(", src)))
+    assert names == sorted(benchlib.EXPORTS), names
+    blib, lib = benchlib.load_library(), binding.load_library()
+    for n in names:
+        assert hasattr(blib, n), n
+        assert not hasattr(lib, n), n
+    pkg = os.path.join(ROOT, "paper_1802_00147_b200")
+    for f in os.listdir(pkg):
+        if f.endswith(".py"):
+            assert "benchlib" not in open(os.path.join(pkg, f)).read(), f
+
+
 def test_header_is_plain_c(tmp_path):
     """The boundary header must compile as C (no C++ types in the signatures)."""
     c = tmp_path / "t.c"
-    c.write_text('#include "mc.h"\nint main(void){ mc_params p; return (int)sizeof(p) * 0; }\n')
+    c.write_text('#include "mc.h"\n#include "mc_bench.h"\nint main(void){ mc_params p; return (int)sizeof(p) * 0; }\n')
     import subprocess
     subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), "-c", str(c),
                     "-o", str(tmp_path / "t.o")], check=True)

@@ -462,7 +462,7 @@ def test_classification_agreement_at_1e5_steps_on_a_strided_subgrid(mc):
     assert ((cg == 2) == (co == 2)).mean() >= 0.995                                       # dropped cells
     # FLI values on cells regular on both sides: at t = 1e5 the state divergence between FP64 and long double has
     # grown to ~1e-8..1e-6 on regular orbits, i.e. ~0.01 in FLI; a few weakly chaotic ("sticky") cells still below
-    # the threshold differ more (the full-grid run shows up to 1.6, profiles/r01_full_grid_classification.md), so
+    # the threshold differ more (the full-grid run shows up to 1.6, profiles/r02_full_grid_classification.md), so
     # the bound is on the bulk, with a loose cap on the worst cell.
     reg = (co == 0) & (o.fli < 4.5) & (cg == 0)
     dfli = np.abs(gfli[idx][reg] - o.fli[reg])
@@ -677,19 +677,17 @@ def test_config3_quadrupole_scan_at_full_length_sampled_against_oracle(mc):
     """BASELINE config 3 at full size and full length (314 x 314, beta = 0.8, chi = 0.9, per-orbit kappa in [1, 8], 1e5
     steps), QM on and QM off on identical seeds through the scan front end.  400 cells drawn uniformly from the grid
     are recomputed by the long-double oracle both ways: regular / not-regular agrees on >= 99 % (north_star's bar is on
-    grid cells, so the sample is uniform) and the three classes on >= 97 %.  100 more cells from the strong-field rows
-    (r0 < 18, where every chaotic and dropped cell lives and single cells flip between "chaotic" and "dropped" with the
-    last bits, R19) must agree three-way on >= 90 %.  The
+    grid cells, so the sample is uniform).  100 more cells come from the strong-field rows (r0 < 18, where every chaotic
+    and dropped cell lives and single cells flip between "chaotic" and "dropped" with the last bits, R19).  The three-way
+    agreement is held against the flips of the oracle's own double instance on the same cells (derived bar, below).  The
     class-change matrix QM off -> QM on of the sampled cells is the oracle's up to the cells whose class differs."""
     from paper_1802_00147_b200 import scan
     w_on, w_off = workloads.config3(qm=True), workloads.config3(qm=False)
     assert w_on.n_steps == 100_000 and np.array_equal(w_on.states, w_off.states)
     on, off = scan.run_scan(w_on), scan.run_scan(w_off)
-    rng = np.random.default_rng(8)
-    uni = rng.choice(314 * 314, 400, replace=False)
-    strong = np.setdiff1d(rng.choice(314 * 50, 110, replace=False), uni)[:100]
-    idx = np.concatenate([uni, strong])
-    is_uni = np.arange(idx.size) < uni.size
+    from conftest import config3_sample
+    idx, is_uni = config3_sample()
+    uni, strong = idx[is_uni], idx[~is_uni]
     res = {}
     for name, w, g in (("on", w_on, on), ("off", w_off, off)):
         sub = w.subset(idx)
@@ -709,8 +707,20 @@ def test_config3_quadrupole_scan_at_full_length_sampled_against_oracle(mc):
         # kappa up to 8 one cell in six of this grid is chaotic or dropped (one in eleven for config 2).  So the 99 % bar
         # is asserted on regular vs not-regular, and the three-way agreement is asserted at the level the flips allow.
         assert ((cg == 0) == (co == 0))[is_uni].mean() >= 0.99
-        assert (cg == co)[is_uni].mean() >= 0.97
-        assert (cg == co)[~is_uni].mean() >= 0.90 and ((cg == 0) == (co == 0))[~is_uni].mean() >= 0.97
+        assert ((cg == 0) == (co == 0))[~is_uni].mean() >= 0.97
+        # Three classes: the bar is DERIVED, not a literal.  The oracle's own double instance on the same cells flips
+        # k_dbl of them against its long-double instance (tests/test_oracle_conventions.py pins on CPU that those flips
+        # exist and are chaotic <-> dropped only); the GPU is another double-precision realisation, so its count k_gpu is
+        # a second draw from the same distribution: the two may differ by two standard deviations of a Poisson
+        # difference, 2 sqrt(k_gpu + k_dbl).  Flips that involve "regular" are bounded by the 99 % / 97 % above.
+        od = oracle.integrate(sub.states, 1.0, w.n_steps, 3, shadow_eps=1e-8, precision=oracle.DOUBLE, **sub.params())
+        cd = scan.classes(od.fli, od.status)
+        for part, label in ((is_uni, "uniform"), (~is_uni, "strong-field")):
+            k_gpu, k_dbl = int((cg != co)[part].sum()), int((cd != co)[part].sum())
+            print("config 3 QM %s, %s sample: three-way flips vs long double: GPU %d, oracle double instance %d of %d cells"
+                  % (name, label, k_gpu, k_dbl, int(part.sum())))
+            assert k_gpu - k_dbl <= 2.0 * np.sqrt(k_gpu + k_dbl), (name, label, k_gpu, k_dbl)
+        print("  of the GPU's flips, chaotic <-> dropped: %d of %d" % (sum({int(cg[i]), int(co[i])} == {1, 2} for i in bad), bad.size))
         reg = (co == 0) & (cg == 0) & (o.fli < 4.5)
         d = np.abs(g["fli"].ravel()[idx][reg] - o.fli[reg])
         assert reg.sum() > 300 and np.median(d) < 0.02 and np.quantile(d, 0.99) < 0.2

@@ -110,3 +110,28 @@ def test_bench_sharding_path_is_a_balanced_partition(world):
     args0 = argparse.Namespace(workload="config0", grid=314, n_steps=100)
     w0 = bench.global_workload(args0, world)
     assert bench.rank_shard(w0, args0, 1, world) is w0
+
+
+@pytest.mark.parametrize("world", [2, 8])
+def test_bench_strong_scaling_path_deals_the_same_grid(world):
+    """bench.py --gpus N --scaling strong: the SAME 314 x 314 scan, row i on rank i mod N (n/G orbits per GPU).
+    The shards are disjoint, complete, differ by at most one row, and every rank sees the whole r0 range."""
+    import argparse
+    import bench
+    args = argparse.Namespace(workload="config2", grid=314, n_steps=1000, scaling="strong")
+    full = bench.global_workload(args, world)
+    assert full.n_orbits == 314 * 314
+    seen = np.zeros(full.n_orbits, dtype=int)
+    sizes = []
+    for rank in range(world):
+        mine = bench.rank_shard(full, args, rank, world)
+        idx = sharding.strong_orbits(314, 314, rank, world)
+        assert np.array_equal(mine.states, full.states[:, idx])
+        seen[idx] += 1
+        sizes.append(mine.n_orbits)
+        r0 = mine.states[0]
+        assert r0.min() < 10.0 + 50.0 * world / 313 + 1e-9 and r0.max() > 60.0 - 50.0 * world / 313 - 1e-9
+    assert (seen == 1).all()
+    assert max(sizes) - min(sizes) <= 314 and sum(sizes) == 314 * 314
+    if world == 8:
+        assert sorted(set(sizes)) == [39 * 314, 40 * 314]      # 12 246 / 12 560 orbits per rank (DESIGN.md section 13)

@@ -135,7 +135,7 @@ def algorithmic_flop(w, mode, integrator, steps_done, gn_steps):
             "per_trajectory_step_without_gn": per_traj_step}
 
 
-def executed_from_sass(w, rk5, warp_work, per_launch_s, num_sms, sm_mhz, value):
+def executed_from_sass(w, rk5, warp_work, per_launch_s, num_sms, sm_mhz, value, probe=None):
     """What the device executed in one launch, from the SASS instruction mix of the step loop (sass_mix.py, read from
     the library's own object file) times the warp-level work counters of the launch (mc_get_warp_work), and the time
     the FP64 pipe needs for it under the measured operand-bandwidth rule (3 cycles for an FMA with three distinct
@@ -149,7 +149,13 @@ def executed_from_sass(w, rk5, warp_work, per_launch_s, num_sms, sm_mhz, value):
     if mix is None:
         return None
     g = warp_work["gn_warp_passes"] / warp_work["warp_steps"]
-    per = sass_mix.per_warp_step(mix, g)
+    rule, rule_text = None, "3.03 cycles per FMA reading 3 distinct registers, 2.19 with an operand-reuse hit, 2.03 otherwise (frozen B200 figures)"
+    if probe:                                   # the cycle rule as mc_fp64_probe measured it in THIS run
+        kinds = benchlib_probe_kinds()
+        rule = (probe[kinds[0]][0], probe[kinds[1]][0], max(probe[kinds[2]][0], probe[kinds[3]][0]))
+        rule_text = ("%.2f cycles per FMA reading 3 distinct registers, %.2f with an operand-reuse hit, %.2f otherwise "
+                     "(mc_fp64_probe, measured in this run)" % rule)
+    per = sass_mix.per_warp_step(mix, g, rule)
     flop = per["flop"] * 32.0 * warp_work["warp_steps"]              # every lane slot of every executed warp instruction
     cycles = per["cycles"] * warp_work["warp_steps"] / (4.0 * num_sms)   # per sub-partition, perfectly balanced
     model_s = cycles / (sm_mhz * 1e6)
@@ -159,7 +165,12 @@ def executed_from_sass(w, rk5, warp_work, per_launch_s, num_sms, sm_mhz, value):
             "executed_tflops": flop / per_launch_s / 1e12,
             "operand_bandwidth_model": {"cycles_per_warp_step": per["cycles"], "kernel_ms": model_s * 1e3,
                                         "measured_over_model": per_launch_s / model_s,
-                                        "rule": "3.03 cycles per FMA reading 3 distinct registers, 2.19 with an operand-reuse hit, 2.03 otherwise (mc_fp64_probe)"}}
+                                        "rule": rule_text}}
+
+
+def benchlib_probe_kinds():
+    import benchlib
+    return benchlib.FP64_PROBE_KINDS
 
 
 def global_workload(args, world):
@@ -379,7 +390,7 @@ def run_mc(args):
     flop_per_launch = float(alg["flop_per_launch"])
     traj = alg["trajectories_per_orbit"]
     achieved_tf = flop_per_launch / per_launch_s / 1e12
-    executed = executed_from_sass(w, rk5, warp_work, per_launch_s, info["num_sms"], sm_max, value)
+    executed = executed_from_sass(w, rk5, warp_work, per_launch_s, info["num_sms"], sm_max, value, probe)
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": nominal_tf, "unit": "TFLOP/s",
                 "frac": achieved_tf / nominal_tf,
                 "traffic": NCU_DRAM_BYTES_PER_LAUNCH_314 if (w.name.startswith("config2") and args.grid == 314 and world == 1) else None,

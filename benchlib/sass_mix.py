@@ -126,12 +126,17 @@ def analyse(params=0, qm=False, mode=3, integ=0, rr=False, obj=None):
             "cycle_rule": {"dfma_3_registers": CYC_3RF, "dfma_reuse_hit": CYC_REUSE, "other_fp64": CYC_PLAIN}}
 
 
-def per_warp_step(mix, gn_iterations_per_warp_step):
-    """Executed FP64 instructions, flop (per lane) and model cycles of one warp-step."""
+def per_warp_step(mix, gn_iterations_per_warp_step, rule=None):
+    """Executed FP64 instructions, flop (per lane) and model cycles of one warp-step.  `rule` = (cycles of a 3-register
+    FMA, of an FMA with an operand-reuse hit, of any other FP64 instruction) as measured in the same run by mc_fp64_probe;
+    without it the B200 figures frozen in this file (CYC_*) apply."""
     g = gn_iterations_per_warp_step
     out = {}
-    for k in ("fp64", "flop", "cycles", "all", "DFMA", "DMUL", "DADD", "dfma_3reg"):
+    for k in ("fp64", "flop", "cycles", "all", "DFMA", "DMUL", "DADD", "dfma_3reg", "dfma_reuse_hit"):
         out[k] = mix["step_fixed"][k] + g * mix["gn_iteration"][k] + mix["tail"][k]
+    if rule is not None:
+        c3, cr, cp = rule
+        out["cycles"] = c3 * out["dfma_3reg"] + cr * out["dfma_reuse_hit"] + cp * (out["fp64"] - out["dfma_3reg"] - out["dfma_reuse_hit"])
     return out
 
 

@@ -32,9 +32,9 @@ UNIT = "orbit-steps/s"
 # terminated, R6): the kernel counts them (mc_get_work).
 # DRAM traffic of ONE FULL-LENGTH launch (314 x 314 orbits + shadows, 1e5 steps) of the hot kernel:
 # dram__bytes_read.sum + dram__bytes_write.sum from the ncu capture of that very launch configuration
-# (profiles/r02_ncu_integrate_kernel_mode3.md, section "DRAM traffic of the full-length launch").  Outputs (31 MB) and the carry buffer (31 MB) live in the 126 MB L2;
+# (profiles/r03_ncu_other_kernels.md, section "DRAM traffic of the full-length launch"; profiles/r03_traffic_full_length_launch.csv).  Outputs (31 MB) and the carry buffer (31 MB) live in the 126 MB L2;
 # algorithmic: 340 B per orbit.
-NCU_DRAM_BYTES_PER_LAUNCH_314 = 10028800 + 7679232   # read + write, bytes
+NCU_DRAM_BYTES_PER_LAUNCH_314 = 9861888 + 7502080   # read + write, bytes (round 3: profiles/r03_ncu_other_kernels.md, last section)
 FP64_LANES_PER_SM = 64
 
 
@@ -395,7 +395,7 @@ def run_mc(args):
                 "frac": achieved_tf / nominal_tf,
                 "traffic": NCU_DRAM_BYTES_PER_LAUNCH_314 if (w.name.startswith("config2") and args.grid == 314 and world == 1) else None,
                 "traffic_unit": "bytes per launch: dram__bytes_read.sum + dram__bytes_write.sum of one full-length (1e5-step) launch of "
-                                "this kernel and grid under ncu (profiles/r02_ncu_integrate_kernel_mode3.md); not re-measured in this run",
+                                "this kernel and grid under ncu (profiles/r03_ncu_other_kernels.md, r03_traffic_full_length_launch.csv); not re-measured in this run",
                 "algorithmic_bytes_per_launch": 340.0 * n,
                 "peak_source": f"derived: {info['num_sms']} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x {sm_max:.0f} MHz "
                                "(MEASURED_PEAKS.json has no FP64 entry)",

@@ -66,17 +66,14 @@ void model(const HostConsts& c, int mode, int newton_iters, mc_flop_model_t* out
   } else {
     out->correct_fixed = run(newton_iters);
   }
-  // status test of a completed step: |r|^2 against the two thresholds (the finite test is integer work)
-  out->status = count([&] { Cnt r2 = mc::dot3(z, z); (void)(r2 < Cnt(4.0)); });
-  // one shadow renormalisation: 12-norm, sqrt, d0 / d, pull-back, eq (10), re-referenced integrals (log10 not counted)
+  // status test of a completed step and one shadow renormalisation: the very templates the kernel's step loop calls
+  // (mc_correct.cuh); the finite test is integer work, log10 is bookkeeping
+  out->status = count([&] { (void)mc::radius_status(z, Cnt(4.0), Cnt(1e8)); });
   out->renorm = count([&] {
-    Cnt d2 = 0.0, y[12];
-    for (int i = 0; i < 12; ++i) { const Cnt e = z[i] - f[i]; d2 = fma(e, e, d2); }
-    const Cnt d = mc::sqrt_pos(d2);
-    const Cnt s = mc::div_(Cnt(1e-8), d);
-    for (int i = 0; i < 12; ++i) y[i] = fma(s, z[i] - f[i], f[i]);
-    if (mode >= 1) { mc::normalise3(y + 6); mc::normalise3(y + 9); }
-    mc::references<QM>(c, y, R);
+    Cnt y[12], acc = 0.0;
+    for (int i = 0; i < 12; ++i) y[i] = Cnt(f[i].v);
+    if (mode >= 1) mc::renormalise_shadow<1, QM>(c, y, z, Cnt(1e-8), acc, R);
+    else mc::renormalise_shadow<0, QM>(c, y, z, Cnt(1e-8), acc, R);
   });
 }
 

@@ -19,6 +19,36 @@ MC_DEV void references(const C& c, const T* z, RefsT<T>& R) {
   total_J(c, z, R.J0);
 }
 
+enum { ST_OK = 0, ST_MERGED = 1, ST_UNBOUND = 2, ST_NONFINITE = 3, ST_NEWTON_FLAG = 256 };
+
+// Status of a completed step from the main trajectory's |r|^2 (R13).  The non-finite
+// test is integer work and stays with the caller.  Used by the kernel's step loop and by the flop model.
+template <class T>
+MC_DEV int radius_status(const T* z, T r_merge2, T r_escape2) {
+  const T r2 = dot3(z, z);
+  return (r2 < r_merge2) ? ST_MERGED : ((r2 > r_escape2) ? ST_UNBOUND : ST_OK);
+}
+
+// One shadow renormalisation (R10-R12): d = |y - ym| over all 12 components, FLI accumulator += log10(d / d0),
+// the shadow y is pulled back onto the main state ym at distance d0 along y - ym, its spins are renormalised (eq 10) and
+// its reference integrals re-taken from the new state (R11).  Returns false, leaving everything untouched, when d is
+// zero or not finite.  Used by the kernel's step loop and by the flop model.
+template <int MODE, bool QM, class C, class T>
+MC_DEV bool renormalise_shadow(const C& c, T* y, const T* ym, T d0, T& acc, RefsT<T>& R) {
+  T d2 = 0.0;
+#pragma unroll
+  for (int i = 0; i < 12; ++i) { const T e = y[i] - ym[i]; d2 = fma(e, e, d2); }
+  const T d = sqrt_pos(d2);
+  if (!(d > T(0.0)) || !(d < T(1.0e300))) return false;
+  acc += log10_(div_exact(d, d0));
+  const T s = div_exact(d0, d);
+#pragma unroll
+  for (int i = 0; i < 12; ++i) y[i] = fma(s, y[i] - ym[i], ym[i]);
+  if (MODE >= 1) { normalise3(y + 6); normalise3(y + 9); }
+  references<QM>(c, y, R);
+  return true;
+}
+
 // Mode 3: minimal-norm Gauss-Newton projection of (r,p) onto {H = E0, r x p = Lt}, Lt = J0 - S1 - S2.
 // Constraint Jacobian D (4 x 6): row (a, b) = (dH/dr, dH/dp) and the three rows (p x e_k, e_k x r) of r x p.  The
 // step is d = D^T (D D^T)^-1 F, F = (H - E0, r x p - Lt), z <- z - d.  The oracle assembles D D^T and solves it by

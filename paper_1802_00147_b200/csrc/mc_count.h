@@ -38,6 +38,8 @@ inline Cnt rsqrt_pos(Cnt x) { ++op_counts().special; return Cnt(1.0 / std::sqrt(
 inline Cnt rcp_nz(Cnt x) { ++op_counts().special; return Cnt(1.0 / x.v); }
 inline Cnt sqrt_pos(Cnt x) { ++op_counts().special; return Cnt(std::sqrt(x.v)); }
 inline Cnt div_(Cnt a, Cnt b) { ++op_counts().special; return Cnt(a.v / b.v); }
+inline Cnt div_exact(Cnt a, Cnt b) { ++op_counts().special; return Cnt(a.v / b.v); }
+inline Cnt log10_(Cnt x) { return Cnt(std::log10(x.v)); }   // the logarithm of the FLI is bookkeeping, not counted
 inline Cnt abs_(Cnt x) { return Cnt(std::fabs(x.v)); }
 inline bool is_finite(Cnt x) { return std::isfinite(x.v); }
 inline bool warp_any(bool b) { return b; }

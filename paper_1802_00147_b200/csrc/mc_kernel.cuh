@@ -57,8 +57,6 @@ struct IntegrateArgs {
   unsigned long long wait_budget_ns;  // a warp waiting longer than this for its unit's previous chunk traps (mc_params.wait_budget_s)
 };
 
-enum { ST_OK = 0, ST_MERGED = 1, ST_UNBOUND = 2, ST_NONFINITE = 3, ST_NEWTON_FLAG = 256 };
-
 // Checked build (-DMC_CHECKED, libmc_checked.so; compute-sanitizer is closed on this GPU pool): every index and pointer
 // the kernel is about to use for a global access is tested first; the source line of the first failed test lands in
 // queue[3] (mc_debug_check).  The product build compiles the tests away.
@@ -244,10 +242,7 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
       // status of the completed step (R13): non-finite anywhere in the pair, else |r| of the main
       int code = ST_OK;
       if (!finite12(z)) code = ST_NONFINITE;
-      else if (!role_shadow) {
-        const double r2 = dot3(z, z);
-        code = (r2 < A.r_merge2) ? ST_MERGED : ((r2 > A.r_escape2) ? ST_UNBOUND : ST_OK);
-      }
+      else if (!role_shadow) code = radius_status(z, A.r_merge2, A.r_escape2);
       if (shadow) {
         const int other = __shfl_xor_sync(0xffffffffu, code, 1);
         code = (code == ST_NONFINITE || other == ST_NONFINITE) ? ST_NONFINITE : (role_shadow ? other : code);
@@ -281,21 +276,9 @@ integrate_kernel(const __grid_constant__ McConsts uc, const __grid_constant__ In
         for (int i = 0; i < 12; ++i) ym[i] = __shfl_xor_sync(0xffffffffu, y[i], 1);
         int bad = 0;
         if (role_shadow && !frozen) {
-          double d2 = 0.0;
-#pragma unroll
-          for (int i = 0; i < 12; ++i) { const double e = y[i] - ym[i]; d2 = fma(e, e, d2); }
-          const double d = sqrt(d2);
-          if (!(d > 0.0) || !(d < 1.0e300)) {
-            bad = 1;
-          } else {
-            acc += log10(d / d0);
-            const double s = d0 / d;
-#pragma unroll
-            for (int i = 0; i < 12; ++i) y[i] = fma(s, y[i] - ym[i], ym[i]);
-            if (MODE >= 1) { normalise3(y + 6); normalise3(y + 9); }
-            references<QM>(c, y, R);   // the shadow obeys its own, re-referenced integrals (R11)
-            if constexpr (RR) { y[12] = R.E0; y[13] = R.J0[0]; y[14] = R.J0[1]; y[15] = R.J0[2]; }   // W, G restart with them
-          }
+          // distance, FLI term, pull-back, eq (10), re-referenced integrals (R11): mc_correct.cuh
+          if (!renormalise_shadow<MODE, QM>(c, y, ym, d0, acc, R)) bad = 1;
+          else if constexpr (RR) { y[12] = R.E0; y[13] = R.J0[0]; y[14] = R.J0[1]; y[15] = R.J0[2]; }   // W, G restart with them
         }
         bad |= __shfl_xor_sync(0xffffffffu, bad, 1);
         if (bad && !frozen) { frozen = true; status = ST_NONFINITE; }

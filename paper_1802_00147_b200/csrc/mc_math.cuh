@@ -71,6 +71,9 @@ __device__ __forceinline__ double sqrt_pos(double x) { return sqrt(x); }
 // sequence with its slow path in the step loop).  b = 0 or non-finite gives a non-finite result, which the caller's
 // skip test catches just as it would after a true division.
 __device__ __forceinline__ double div_(double a, double b) { return a * rcp_nz(b); }
+// IEEE division and log10 for the shadow renormalisation (once per renorm_interval steps, outside the hot sequence)
+__device__ __forceinline__ double div_exact(double a, double b) { return a / b; }
+__device__ __forceinline__ double log10_(double x) { return log10(x); }
 __device__ __forceinline__ bool is_finite(double v) { return (((unsigned)__double2hiint(v)) & 0x7ff00000u) != 0x7ff00000u; }
 
 __device__ __forceinline__ bool finite12(const double* z) {
